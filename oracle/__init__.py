@@ -1,0 +1,13 @@
+"""CPU oracle for the VIPIR database scan -- TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product
+(``paper_2606_11536_b200``) never does, and this package never imports the product.
+"""
+from .vipir_oracle import (  # noqa: F401
+    build,
+    dbmul,
+    dbmul_limbs,
+    dbmul_bruteforce,
+    lib_path,
+)
