@@ -1,0 +1,154 @@
+/*
+ * vipir.h -- C ABI of libvipir: the VIPIR PIR server's database scan on one B200.
+ *
+ *     answer = D * Q  mod q
+ *
+ * the "D1 x B x D0 INT8-INT32 GEMM for a batch of B queries" that is the server's online
+ * step (arxiv/paper_2606_11536, section 2.5), with the plaintext database
+ * D (rows x cols small unsigned integers) and the encrypted query matrix Q (u32 words).
+ * Modulus: q = 2^32, "modulo-2^32 operations as in SimplePIR ... modular reduction
+ * effectively becomes free" (section 4), or per-prime RNS residues, "each row
+ * corresponds to a different q_i" (section 2.3).  The method is the paper's
+ * limb decomposition A*B = sum_j 2^(8j) (A*B_j) over 8-bit query limbs (PAPER.md:245-249
+ * section 4.1) on int8 tensor cores (batched) or CUDA cores (batch 1).
+ *
+ * Definition of the result (bit-exact; no tolerance).  For modulus index t < T, query b < batch,
+ * row r < rows:
+ *     answer[t][b][r] = ( sum_{k < cols} D[r][k] * Q[t][b][k] )  mod q_t
+ * D[r][k] the UNSIGNED value of the element, Q the unsigned 32-bit word (any u32 is legal,
+ * also >= q_t), the sum over the integers, the result canonical in [0, q_t).
+ * T = max(mod.count, 1); mod.count == 0 selects q = 2^32.
+ *
+ * Layouts (all dense, no pitch):
+ *   d_db      rows x cols, row-major (cols contiguous), uint8, or little-endian uint16 when
+ *             db_bits == 16.  DEVICE pointer, 16-byte aligned.  cols * db_bits/8 must be a
+ *             multiple of 16 bytes.
+ *   d_query   [T][batch][cols] uint32 -- each query vector contiguous.  DEVICE pointer, 16-byte aligned.
+ *   d_answer  [T][batch][rows] uint32.  DEVICE pointer.
+ * Ownership: the caller owns d_db, d_query, d_answer (they must not overlap and must stay
+ * valid until the stream has run the call); the plan owns its workspace (query limb planes,
+ * host-call staging) and frees it in vipir_destroy.
+ *
+ * Execution: vipir_dbmul only ENQUEUES work on `cuda_stream` (a cudaStream_t / CUstream passed
+ * as void*, NULL = legacy default stream): no host synchronisation, no allocation.  One plan
+ * must not be in flight on two streams at once (shared workspace).  All kernels are sm_100a;
+ * there is no fallback of any kind.
+ *
+ * Errors: every entry point returns a vipir_status (0 = OK) and never throws or aborts.
+ */
+#ifndef VIPIR_H
+#define VIPIR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vipir_plan vipir_plan; /* opaque, owned by the library */
+
+typedef enum {
+    VIPIR_OK = 0,
+    VIPIR_ERR_INVALID_ARG = 1, /* null pointer, zero size, db_bits not 8/16, modulus < 2 or >= 2^30, count > 4 */
+    VIPIR_ERR_UNSUPPORTED = 2, /* row bytes not a multiple of 16, size beyond a stated limit, regime cannot run this shape */
+    VIPIR_ERR_ALLOC = 3,       /* host or device allocation failed */
+    VIPIR_ERR_CUDA = 4,        /* a CUDA call failed (no device, launch error, ...) */
+    VIPIR_ERR_ARCH = 5         /* the current device is not compute capability 10.0 (B200) */
+} vipir_status;
+
+#define VIPIR_MAX_MODULI 4u
+
+typedef struct {
+    uint32_t count;         /* 0 => q = 2^32 (wrapping); else number of moduli (<= VIPIR_MAX_MODULI) */
+    const uint32_t *moduli; /* HOST pointer to `count` values, each 2 <= m < 2^30; copied by the plan */
+} vipir_modulus_spec;
+
+/* Kernel regimes.  AUTO picks GEMV for one wrapping query vector,
+ * otherwise the tensor-core path (1-SM tiles while the product is HBM-bound, 2-SM pairs
+ * above).  NAIVE is a test-only check kernel and is never picked by AUTO. */
+typedef enum {
+    VIPIR_REGIME_AUTO = 0,
+    VIPIR_REGIME_GEMV = 1,    /* step a2: CUDA-core dp4a scan, batch 1, q = 2^32 only */
+    VIPIR_REGIME_MMA_1SM = 2, /* steps a3-a5: tcgen05.mma.cta_group::1.kind::i8 */
+    VIPIR_REGIME_MMA_2SM = 3, /* steps a3-a5: tcgen05.mma.cta_group::2.kind::i8, CTA pairs */
+    VIPIR_REGIME_NAIVE = 4
+} vipir_regime;
+
+typedef struct {
+    uint32_t regime;          /* the regime in effect (never AUTO) */
+    uint32_t db_limbs;        /* dl: 1 (u8) or 2 (u16) */
+    uint32_t limb_cols;       /* LC: accumulator columns per query vector (4, or 5 for u16 + prime) */
+    uint32_t query_vectors;   /* T * batch */
+    uint64_t k_bytes;         /* K' = cols * dl: bytes per DB row */
+    uint32_t k_chunk_bytes;   /* K' bytes per int32 accumulation chunk (<= 32768); 0 for GEMV/NAIVE */
+    uint32_t n_chunks;
+    uint32_t tile_queries;    /* query vectors per N tile (MMA regimes) */
+    uint32_t tile_cols;       /* accumulator columns per tile = tile_queries * LC */
+    uint32_t mma_n;           /* N of one tcgen05.mma */
+    uint32_t m_tiles, n_tiles;
+    uint32_t stages;          /* shared-memory ring depth */
+    uint32_t smem_bytes;      /* dynamic shared memory per CTA */
+    uint32_t grid;            /* CTAs launched by the main kernel */
+    uint32_t launches;        /* kernels enqueued per vipir_dbmul call */
+    uint64_t workspace_bytes; /* limb planes */
+    void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
+} vipir_info;
+
+/*
+ * Build a plan for one problem shape (host only; allocates the limb-plane workspace on the
+ * current device and picks regime, tiles and K chunks).  SimplePIR shapes: rows = D1,
+ * cols = D0, batch = B.
+ *   out      receives the plan (NULL on failure)
+ *   db_bits  8 or 16
+ *   mod      NULL or count == 0 for q = 2^32
+ * Errors: INVALID_ARG, UNSUPPORTED (cols*db_bits/8 % 16 != 0; rows or cols*db_bits/8 >= 2^31;
+ * T*batch*5 >= 2^31), ARCH, ALLOC, CUDA.
+ */
+int vipir_dbmul_plan(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                     const vipir_modulus_spec *mod);
+
+/* Same, forcing a regime (tests, benchmarks).  UNSUPPORTED if the regime cannot run the shape
+ * (GEMV needs T*batch == 1 and q = 2^32). */
+int vipir_dbmul_plan_ex(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                        const vipir_modulus_spec *mod, uint32_t regime);
+
+/*
+ * Enqueue answer = D * Q mod q on `cuda_stream`: the query-limb splitter
+ * followed by the scan kernel of the plan's regime.  All three pointers are DEVICE pointers.
+ * Errors: INVALID_ARG (null / misaligned pointer), CUDA.
+ */
+int vipir_dbmul(vipir_plan *plan, const void *d_db, const uint32_t *d_query, uint32_t *d_answer,
+                void *cuda_stream);
+
+/*
+ * End-to-end variant with HOST query and answer buffers (the PIR server's per-request path:
+ * queries arrive from clients, answers go back; the static DB stays resident on the GPU,
+ * PAPER.md:176).  Copies h_query to the device, runs vipir_dbmul, copies the answer back and
+ * waits for the stream.  h_query / h_answer: HOST pointers with the d_query / d_answer
+ * layouts (pinned memory makes the copies asynchronous); d_db: DEVICE pointer.  The first
+ * call allocates device staging owned by the plan.
+ */
+int vipir_dbmul_host(vipir_plan *plan, const void *d_db, const uint32_t *h_query, uint32_t *h_answer,
+                     void *cuda_stream);
+
+/* Run only the query-limb splitter (step a1): d_query [T*batch][cols] u32 ->
+ * byte planes [T*batch*LC][K'] u8 (layout: csrc/split_limbs.cuh) written to d_planes_out
+ * (DEVICE, 16-byte aligned, workspace_bytes long), or into the plan's workspace if NULL. */
+int vipir_split_limbs(vipir_plan *plan, const uint32_t *d_query, uint8_t *d_planes_out, void *cuda_stream);
+
+/* Describe the plan.  Errors: INVALID_ARG. */
+int vipir_plan_info(const vipir_plan *plan, vipir_info *out);
+
+/* Free the plan and its workspace.  vipir_destroy(NULL) is a no-op. */
+void vipir_destroy(vipir_plan *plan);
+
+/* Static string for a status code. */
+const char *vipir_status_str(int status);
+
+/* Last CUDA error string recorded by this library on the calling thread ("" if none). */
+const char *vipir_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VIPIR_H */

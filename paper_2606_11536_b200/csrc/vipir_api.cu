@@ -1,0 +1,433 @@
+// vipir_api.cu -- host side of libvipir: plan (step a0), dispatch, C ABI (include/vipir.h).
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "../../include/vipir.h"
+#include "gemm_i8_tcgen05.cuh"
+#include "gemv_b1.cuh"
+#include "naive.cuh"
+#include "split_limbs.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+int cuda_fail(cudaError_t e, const char* where) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", where, cudaGetErrorString(e));
+    return VIPIR_ERR_CUDA;
+}
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);      \
+    } while (0)
+
+constexpr uint32_t kMaxSmem = 232448;  // 227 KiB opt-in dynamic shared memory per CTA
+constexpr uint32_t kChunkBytes = 32768; // 255*255*32768 < 2^31 (R7)
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// 2-D row-major tensor [dim1][dim0] of `esize`-byte elements, row pitch `pitch` bytes.
+int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint32_t esize, uint64_t dim0,
+                 uint64_t dim1, uint64_t pitch, uint32_t box0, uint32_t box1, CUtensorMapSwizzle sw) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled entry point not found");
+        return VIPIR_ERR_CUDA;
+    }
+    cuuint64_t dims[2] = {dim0, dim1};
+    cuuint64_t strides[1] = {pitch};
+    cuuint32_t box[2] = {box0, box1};
+    cuuint32_t estr[2] = {1, 1};
+    (void)esize;
+    CUresult r = fn(m, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
+        return VIPIR_ERR_CUDA;
+    }
+    return VIPIR_OK;
+}
+
+uint32_t round_up(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
+uint32_t ceil_div(uint32_t x, uint32_t m) { return (x + m - 1) / m; }
+
+}  // namespace
+
+struct vipir_plan {
+    uint64_t rows, cols, kbytes;
+    uint32_t batch, db_bits, dl, lc, nq, n_moduli;
+    uint32_t moduli[VIPIR_MAX_MODULI];
+    uint32_t regime;
+    int num_sms;
+    // workspace
+    uint8_t* d_planes;
+    uint64_t planes_bytes;
+    // host-call staging
+    uint32_t* d_q_stage;
+    uint32_t* d_a_stage;
+    // kernel parameters
+    vipir::GemmParams gm;
+    vipir::GemvParams gv;
+    uint32_t smem_bytes, grid;
+    // tensor maps
+    CUtensorMap tm_planes;
+    CUtensorMap tm_db;
+    const void* tm_db_for;  // d_db the cached tm_db was encoded for
+};
+
+namespace {
+
+template <int CG, int LC, bool PRIME>
+int launch_gemm(vipir_plan* p, cudaStream_t st) {
+    auto kern = vipir::gemm_i8_kernel<CG, LC, PRIME>;
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p->grid);
+    cfg.blockDim = dim3(vipir::GM_THREADS);
+    cfg.dynamicSmemBytes = p->smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_db, p->tm_planes, p->gm));
+    return VIPIR_OK;
+}
+
+template <int CG>
+int launch_gemm_cg(vipir_plan* p, cudaStream_t st) {
+    const bool prime = p->n_moduli > 0;
+    if (p->lc == 5) return launch_gemm<CG, 5, true>(p, st);
+    return prime ? launch_gemm<CG, 4, true>(p, st) : launch_gemm<CG, 4, false>(p, st);
+}
+
+int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaStream_t st) {
+    const uint64_t groups = ((p->cols + 15) / 16) * p->nq;
+    const uint32_t blocks = (uint32_t)((groups + 255) / 256);
+    if (p->dl == 1)
+        vipir::split_limbs_kernel<1, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+    else if (p->lc == 4)
+        vipir::split_limbs_kernel<2, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+    else
+        vipir::split_limbs_kernel<2, 5><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+    CK(cudaGetLastError());
+    return VIPIR_OK;
+}
+
+// ---- planning ------------------------------------------------------------------------------
+
+int plan_gemm(vipir_plan* p, int cg) {
+    vipir::GemmParams& g = p->gm;
+    memset(&g, 0, sizeof g);
+    const uint32_t lc = p->lc;
+    const uint32_t bn_max = (cg == 1) ? 256u : 512u;
+    const uint32_t q_align = (lc == 5) ? 16u : 4u;       // keeps bn a multiple of 16 and of 4*LC
+    const uint32_t q_align2 = (lc == 5) ? 32u : 8u;      // two instructions: bn/2 a multiple of 16
+    const uint32_t qt_max = (bn_max / lc) / q_align2 * q_align2;
+    uint32_t qt = round_up(p->nq, q_align);
+    uint32_t n_tiles = 1;
+    if (qt > qt_max) {
+        n_tiles = ceil_div(p->nq, qt_max);
+        qt = round_up(ceil_div(p->nq, n_tiles), q_align);
+    }
+    uint32_t bn = qt * lc;
+    if (bn > 256) {
+        qt = round_up(qt, q_align2);
+        bn = qt * lc;
+    }
+    if (bn > bn_max) return VIPIR_ERR_UNSUPPORTED;
+    g.rows = p->rows;
+    g.nq = p->nq;
+    g.batch = p->batch;
+    g.qt = qt;
+    g.bn = bn;
+    g.n_tiles = ceil_div(p->nq, qt);
+    g.m_tiles = (uint32_t)((p->rows + 128ull * cg - 1) / (128ull * cg));
+    g.n_instr = (bn > 256) ? 2u : 1u;
+    g.ni_cols = bn / g.n_instr;
+    g.total_ksteps = (uint32_t)((p->kbytes + vipir::GM_BK - 1) / vipir::GM_BK);
+    const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
+    g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
+    g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
+    g.stage_bytes = vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
+    const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
+    uint32_t stages = (kMaxSmem - overhead) / g.stage_bytes;
+    if (stages > 12) stages = 12;
+    if (stages < 2) return VIPIR_ERR_UNSUPPORTED;
+    g.stages = stages;
+    g.acc_stages = (2 * bn <= 512) ? 2u : 1u;
+    uint32_t cols_needed = g.acc_stages * bn, tc = 32;
+    while (tc < cols_needed) tc <<= 1;
+    g.tmem_cols = tc;
+    g.idesc = (2u << 4) /* D = s32 */ | (0u << 7) /* A = u8 */ | (0u << 10) /* B = u8 */ |
+              ((g.ni_cols >> 3) << 17) | (((128u * cg) >> 4) << 24);
+    g.n_moduli = p->n_moduli;
+    for (uint32_t t = 0; t < p->n_moduli; ++t) {
+        g.moduli[t] = p->moduli[t];
+        g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / p->moduli[t]);
+    }
+    p->smem_bytes = stages * g.stage_bytes + overhead;
+    const uint32_t units = g.m_tiles * g.n_tiles;
+    const uint32_t max_units = (uint32_t)p->num_sms / cg;
+    p->grid = (units < max_units ? units : max_units) * cg;
+    // limb-plane tensor map: [nq*LC][K'] bytes, box 128 B x (ni_cols / cg) rows, 128B swizzle
+    return make_tmap_2d(&p->tm_planes, p->d_planes, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes,
+                        (uint64_t)p->nq * lc, p->kbytes, vipir::GM_BK, g.ni_cols / cg, CU_TENSOR_MAP_SWIZZLE_128B);
+}
+
+int plan_gemv(vipir_plan* p) {
+    if (p->nq != 1 || p->n_moduli != 0 || p->lc != 4) return VIPIR_ERR_UNSUPPORTED;
+    vipir::GemvParams& g = p->gv;
+    memset(&g, 0, sizeof g);
+    g.rows = p->rows;
+    g.kbytes = (uint32_t)p->kbytes;
+    g.n_ksteps = (uint32_t)((p->kbytes + vipir::GV_KT - 1) / vipir::GV_KT);
+    g.n_blocks = (uint32_t)((p->rows + vipir::GV_R - 1) / vipir::GV_R);
+    g.stages = 6;
+    p->smem_bytes = g.stages * vipir::GV_STAGE_BYTES + 128 + 2 * 8 * g.stages + 2 * vipir::GV_R * 4;
+    p->grid = g.n_blocks < (uint32_t)p->num_sms ? g.n_blocks : (uint32_t)p->num_sms;
+    // limb planes [4][K'] viewed as u32 elements: box 256 elements (1024 B) x 4 rows
+    return make_tmap_2d(&p->tm_planes, p->d_planes, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, p->kbytes / 4, 4, p->kbytes,
+                        vipir::GV_KT / 4, 4, CU_TENSOR_MAP_SWIZZLE_NONE);
+}
+
+int encode_db_map(vipir_plan* p, const void* d_db) {
+    if (p->tm_db_for == d_db) return VIPIR_OK;
+    int rc;
+    if (p->regime == VIPIR_REGIME_GEMV)
+        rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, p->kbytes / 4, p->rows, p->kbytes,
+                          vipir::GV_KT / 4, vipir::GV_R, CU_TENSOR_MAP_SWIZZLE_NONE);
+    else
+        rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes, p->rows, p->kbytes,
+                          vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (rc == VIPIR_OK) p->tm_db_for = d_db;
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* vipir_status_str(int s) {
+    switch (s) {
+        case VIPIR_OK: return "VIPIR_OK";
+        case VIPIR_ERR_INVALID_ARG: return "VIPIR_ERR_INVALID_ARG";
+        case VIPIR_ERR_UNSUPPORTED: return "VIPIR_ERR_UNSUPPORTED";
+        case VIPIR_ERR_ALLOC: return "VIPIR_ERR_ALLOC";
+        case VIPIR_ERR_CUDA: return "VIPIR_ERR_CUDA";
+        case VIPIR_ERR_ARCH: return "VIPIR_ERR_ARCH";
+        default: return "VIPIR_ERR_UNKNOWN";
+    }
+}
+
+const char* vipir_last_cuda_error(void) { return g_cuda_err; }
+
+int vipir_dbmul_plan_ex(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                        const vipir_modulus_spec* mod, uint32_t regime) {
+    if (!out) return VIPIR_ERR_INVALID_ARG;
+    *out = nullptr;
+    // ---- argument checks first: these need no device ----
+    if (rows == 0 || cols == 0 || batch == 0) return VIPIR_ERR_INVALID_ARG;
+    if (db_bits != 8 && db_bits != 16) return VIPIR_ERR_INVALID_ARG;
+    if (regime > VIPIR_REGIME_NAIVE) return VIPIR_ERR_INVALID_ARG;
+    const uint32_t n_moduli = mod ? mod->count : 0;
+    if (n_moduli > VIPIR_MAX_MODULI) return VIPIR_ERR_INVALID_ARG;
+    if (n_moduli > 0 && !mod->moduli) return VIPIR_ERR_INVALID_ARG;
+    for (uint32_t t = 0; t < n_moduli; ++t)
+        if (mod->moduli[t] < 2 || mod->moduli[t] >= (1u << 30)) return VIPIR_ERR_INVALID_ARG;
+    const uint32_t dl = db_bits / 8;
+    if (cols > (1ull << 31) || (cols * dl) % 16 != 0) return VIPIR_ERR_UNSUPPORTED;
+    const uint64_t kbytes = cols * dl;
+    if (rows >= (1ull << 31) || kbytes >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    const uint32_t T = n_moduli ? n_moduli : 1;
+    if ((uint64_t)T * batch * 5 >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+
+    // ---- device ----
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    int major = 0, minor = 0, sms = 0;
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CK(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10 || minor != 0) return VIPIR_ERR_ARCH;
+
+    vipir_plan* p = new (std::nothrow) vipir_plan;
+    if (!p) return VIPIR_ERR_ALLOC;
+    memset(p, 0, sizeof *p);
+    p->rows = rows;
+    p->cols = cols;
+    p->kbytes = kbytes;
+    p->batch = batch;
+    p->db_bits = db_bits;
+    p->dl = dl;
+    p->n_moduli = n_moduli;
+    for (uint32_t t = 0; t < n_moduli; ++t) p->moduli[t] = mod->moduli[t];
+    p->nq = T * batch;
+    p->lc = (dl == 2 && n_moduli > 0) ? 5u : 4u;  // split_limbs.cuh: the s = 4 column vanishes mod 2^32
+    p->num_sms = sms;
+
+    if (regime == VIPIR_REGIME_AUTO) {
+        if (p->nq == 1 && n_moduli == 0) regime = VIPIR_REGIME_GEMV;
+        else regime = ((uint64_t)p->nq * p->lc > 256 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
+    }
+    p->regime = regime;
+
+    p->planes_bytes = (uint64_t)p->nq * p->lc * kbytes;
+    if (cudaMalloc(&p->d_planes, p->planes_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        delete p;
+        return VIPIR_ERR_ALLOC;
+    }
+    int rc = VIPIR_OK;
+    switch (regime) {
+        case VIPIR_REGIME_GEMV: rc = plan_gemv(p); break;
+        case VIPIR_REGIME_MMA_1SM: rc = plan_gemm(p, 1); break;
+        case VIPIR_REGIME_MMA_2SM: rc = plan_gemm(p, 2); break;
+        case VIPIR_REGIME_NAIVE: p->grid = (uint32_t)((rows + 127) / 128); break;
+        default: rc = VIPIR_ERR_INVALID_ARG;
+    }
+    if (rc != VIPIR_OK) {
+        vipir_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return VIPIR_OK;
+}
+
+int vipir_dbmul_plan(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                     const vipir_modulus_spec* mod) {
+    return vipir_dbmul_plan_ex(out, rows, cols, batch, db_bits, mod, VIPIR_REGIME_AUTO);
+}
+
+int vipir_split_limbs(vipir_plan* p, const uint32_t* d_query, uint8_t* d_planes_out, void* cuda_stream) {
+    if (!p || !d_query || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
+        (reinterpret_cast<uintptr_t>(d_planes_out) & 15))
+        return VIPIR_ERR_INVALID_ARG;
+    return launch_split(p, d_query, d_planes_out ? d_planes_out : p->d_planes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32_t* d_answer, void* cuda_stream) {
+    if (!p || !d_db || !d_query || !d_answer) return VIPIR_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
+        (reinterpret_cast<uintptr_t>(d_answer) & 3))
+        return VIPIR_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+    if (p->regime == VIPIR_REGIME_NAIVE) {
+        vipir::NaiveParams np{};
+        np.rows = p->rows;
+        np.cols = p->cols;
+        np.batch = p->batch;
+        np.db_bits = p->db_bits;
+        np.n_moduli = p->n_moduli;
+        for (uint32_t t = 0; t < p->n_moduli; ++t) np.moduli[t] = p->moduli[t];
+        vipir::naive_dbmul_kernel<<<dim3(p->grid, p->nq), 128, 0, st>>>(d_db, d_query, d_answer, np);
+        CK(cudaGetLastError());
+        return VIPIR_OK;
+    }
+
+    int rc = encode_db_map(p, d_db);
+    if (rc != VIPIR_OK) return rc;
+    rc = launch_split(p, d_query, p->d_planes, st);
+    if (rc != VIPIR_OK) return rc;
+
+    if (p->regime == VIPIR_REGIME_GEMV) {
+        static thread_local bool attr_set = false;
+        if (!attr_set) {
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+            attr_set = true;
+        }
+        p->gv.answer = d_answer;
+        vipir::gemv_b1_kernel<<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        CK(cudaGetLastError());
+        return VIPIR_OK;
+    }
+    p->gm.answer = d_answer;
+    return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
+}
+
+int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, uint32_t* h_answer, void* cuda_stream) {
+    if (!p || !d_db || !h_query || !h_answer) return VIPIR_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t qbytes = (size_t)p->nq * p->cols * 4, abytes = (size_t)p->nq * p->rows * 4;
+    if (!p->d_q_stage) {
+        if (cudaMalloc(&p->d_q_stage, qbytes) != cudaSuccess || cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
+            cudaGetLastError();
+            return VIPIR_ERR_ALLOC;
+        }
+    }
+    CK(cudaMemcpyAsync(p->d_q_stage, h_query, qbytes, cudaMemcpyHostToDevice, st));
+    int rc = vipir_dbmul(p, d_db, p->d_q_stage, p->d_a_stage, cuda_stream);
+    if (rc != VIPIR_OK) return rc;
+    CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return VIPIR_OK;
+}
+
+int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
+    if (!p || !o) return VIPIR_ERR_INVALID_ARG;
+    memset(o, 0, sizeof *o);
+    o->regime = p->regime;
+    o->db_limbs = p->dl;
+    o->limb_cols = p->lc;
+    o->query_vectors = p->nq;
+    o->k_bytes = p->kbytes;
+    o->smem_bytes = p->smem_bytes;
+    o->grid = p->grid;
+    o->workspace_bytes = p->planes_bytes;
+    o->d_limb_planes = p->d_planes;
+    o->launches = (p->regime == VIPIR_REGIME_NAIVE) ? 1 : 2;
+    if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
+        o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;
+        o->n_chunks = p->gm.n_chunks;
+        o->tile_queries = p->gm.qt;
+        o->tile_cols = p->gm.bn;
+        o->mma_n = p->gm.ni_cols;
+        o->m_tiles = p->gm.m_tiles;
+        o->n_tiles = p->gm.n_tiles;
+        o->stages = p->gm.stages;
+    } else if (p->regime == VIPIR_REGIME_GEMV) {
+        o->n_chunks = 1;
+        o->m_tiles = p->gv.n_blocks;
+        o->n_tiles = 1;
+        o->stages = p->gv.stages;
+    }
+    return VIPIR_OK;
+}
+
+void vipir_destroy(vipir_plan* p) {
+    if (!p) return;
+    if (p->d_planes) cudaFree(p->d_planes);
+    if (p->d_q_stage) cudaFree(p->d_q_stage);
+    if (p->d_a_stage) cudaFree(p->d_a_stage);
+    delete p;
+}
+
+}  // extern "C"

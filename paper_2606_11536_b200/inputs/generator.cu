@@ -1,0 +1,58 @@
+// generator.cu -- device twin of generator.py: the same SplitMix64 byte stream and
+// residues, written straight into device memory so that a 16 GiB DB never needs a host
+// copy.  Holds none of the method's arithmetic.  C ABI, loaded by inputs/device.py.
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace {
+
+__device__ __forceinline__ uint64_t word(uint64_t key, uint64_t i) {
+    uint64_t z = key + (i + 1) * 0x9E3779B97F4A7C15ull;
+    z ^= z >> 30;
+    z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27;
+    z *= 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+// dst is 16-byte aligned; word index of dst[0] is word0; n_words words are written
+__global__ void fill_words_kernel(uint64_t* dst, uint64_t n_words, uint64_t key, uint64_t word0) {
+    const uint64_t pairs = n_words / 2;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < pairs; i += stride) {
+        ulonglong2 v;
+        v.x = word(key, word0 + 2 * i);
+        v.y = word(key, word0 + 2 * i + 1);
+        reinterpret_cast<ulonglong2*>(dst)[i] = v;
+    }
+    if ((n_words & 1) && blockIdx.x == 0 && threadIdx.x == 0) dst[n_words - 1] = word(key, word0 + n_words - 1);
+}
+
+__global__ void fill_mod_kernel(uint32_t* dst, uint64_t n, uint64_t key, uint64_t start, uint32_t p) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        dst[i] = (uint32_t)(word(key, start + i) % p);
+}
+
+}  // namespace
+
+extern "C" {
+
+// Bytes [0, nbytes) of the stream `key` into d_dst (device, 16-byte aligned, nbytes % 8 == 0).
+int vipir_inputs_fill_bytes(void* d_dst, uint64_t nbytes, uint64_t key, void* stream) {
+    if (!d_dst || (nbytes & 7) || (reinterpret_cast<uintptr_t>(d_dst) & 15)) return 1;
+    if (nbytes == 0) return 0;
+    fill_words_kernel<<<148 * 8, 256, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<uint64_t*>(d_dst), nbytes / 8,
+                                                                             key, 0);
+    return cudaGetLastError() == cudaSuccess ? 0 : 2;
+}
+
+// word(key, start + i) % p for i < n into d_dst (device u32).
+int vipir_inputs_fill_mod(uint32_t* d_dst, uint64_t n, uint64_t key, uint64_t start, uint32_t p, void* stream) {
+    if (!d_dst || p < 2) return 1;
+    if (n == 0) return 0;
+    fill_mod_kernel<<<148 * 8, 256, 0, static_cast<cudaStream_t>(stream)>>>(d_dst, n, key, start, p);
+    return cudaGetLastError() == cudaSuccess ? 0 : 2;
+}
+
+}  // extern "C"

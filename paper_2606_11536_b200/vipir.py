@@ -1,0 +1,188 @@
+"""Thin ctypes binding of libvipir (include/vipir.h): argument marshalling only.
+
+Every step of the hot path runs inside csrc/libvipir.so; torch is used for device memory and
+streams, nothing else.  There is no CPU fallback: if the shared library is missing or fails
+to load, the first call raises.
+
+    plan = vipir.dbmul_plan(rows, cols, batch, db_bits=8, moduli=None)
+    vipir.dbmul(plan, d_db, d_query, d_answer)          # torch CUDA tensors, current stream
+    vipir.destroy(plan)                                  # or use `with vipir.Plan(...) as p:`
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+_LIB_PATH = Path(__file__).resolve().parent / "csrc" / "libvipir.so"
+_lib = None
+
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_ARCH = range(6)
+REGIME_AUTO, REGIME_GEMV, REGIME_MMA_1SM, REGIME_MMA_2SM, REGIME_NAIVE = range(5)
+REGIME_NAMES = {0: "auto", 1: "gemv", 2: "mma_1sm", 3: "mma_2sm", 4: "naive"}
+MAX_MODULI = 4
+
+# every symbol include/vipir.h declares
+SYMBOLS = (
+    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs",
+    "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
+)
+
+
+class ModulusSpec(ctypes.Structure):
+    _fields_ = [("count", ctypes.c_uint32), ("moduli", ctypes.POINTER(ctypes.c_uint32))]
+
+
+class Info(ctypes.Structure):
+    _fields_ = [
+        ("regime", ctypes.c_uint32), ("db_limbs", ctypes.c_uint32), ("limb_cols", ctypes.c_uint32),
+        ("query_vectors", ctypes.c_uint32), ("k_bytes", ctypes.c_uint64), ("k_chunk_bytes", ctypes.c_uint32),
+        ("n_chunks", ctypes.c_uint32), ("tile_queries", ctypes.c_uint32), ("tile_cols", ctypes.c_uint32),
+        ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32), ("n_tiles", ctypes.c_uint32),
+        ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
+        ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
+    ]
+
+    def as_dict(self):
+        d = {k: getattr(self, k) for k, _ in self._fields_}
+        d["regime_name"] = REGIME_NAMES.get(d["regime"], "?")
+        return d
+
+
+class VipirError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        lib = load()
+        name = lib.vipir_status_str(status).decode()
+        detail = lib.vipir_last_cuda_error().decode() if status == ERR_CUDA else ""
+        super().__init__(f"{what}: {name}" + (f" ({detail})" if detail else ""))
+
+
+def lib_path() -> Path:
+    return _LIB_PATH
+
+
+def load() -> ctypes.CDLL:
+    """Load csrc/libvipir.so; raises if it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2606_11536_b200.build` "
+                               "(the CUDA library is the only implementation; there is no CPU fallback)")
+        lib = ctypes.CDLL(str(_LIB_PATH))
+        u64, u32, vp, i = ctypes.c_uint64, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_int
+        pp = ctypes.POINTER(ctypes.c_void_p)
+        ms = ctypes.POINTER(ModulusSpec)
+        lib.vipir_dbmul_plan.restype = i
+        lib.vipir_dbmul_plan.argtypes = [pp, u64, u64, u32, u32, ms]
+        lib.vipir_dbmul_plan_ex.restype = i
+        lib.vipir_dbmul_plan_ex.argtypes = [pp, u64, u64, u32, u32, ms, u32]
+        lib.vipir_dbmul.restype = i
+        lib.vipir_dbmul.argtypes = [vp, vp, vp, vp, vp]
+        lib.vipir_dbmul_host.restype = i
+        lib.vipir_dbmul_host.argtypes = [vp, vp, vp, vp, vp]
+        lib.vipir_split_limbs.restype = i
+        lib.vipir_split_limbs.argtypes = [vp, vp, vp, vp]
+        lib.vipir_plan_info.restype = i
+        lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
+        lib.vipir_destroy.restype = None
+        lib.vipir_destroy.argtypes = [vp]
+        lib.vipir_status_str.restype = ctypes.c_char_p
+        lib.vipir_status_str.argtypes = [i]
+        lib.vipir_last_cuda_error.restype = ctypes.c_char_p
+        lib.vipir_last_cuda_error.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _check(status: int, what: str):
+    if status != OK:
+        raise VipirError(status, what)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return ctypes.c_void_p(stream)
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor, numpy array or raw int."""
+    if isinstance(t, int):
+        return ctypes.c_void_p(t)
+    if hasattr(t, "data_ptr"):
+        return ctypes.c_void_p(t.data_ptr())
+    return ctypes.c_void_p(t.ctypes.data)
+
+
+def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, regime: int = REGIME_AUTO):
+    """vipir_dbmul_plan[_ex]; returns the opaque plan handle (a c_void_p)."""
+    lib = load()
+    handle = ctypes.c_void_p()
+    spec_p = None
+    if moduli is not None and len(moduli) > 0:
+        arr = (ctypes.c_uint32 * len(moduli))(*[int(m) for m in moduli])
+        spec = ModulusSpec(len(moduli), arr)
+        spec_p = ctypes.byref(spec)
+    _check(lib.vipir_dbmul_plan_ex(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime), "vipir_dbmul_plan")
+    return handle
+
+
+def dbmul(plan, d_db, d_query, d_answer, stream=None):
+    """vipir_dbmul: enqueue answer = D*Q mod q on `stream` (default: torch's current stream)."""
+    _check(load().vipir_dbmul(plan, _ptr(d_db), _ptr(d_query), _ptr(d_answer), _stream_ptr(stream)), "vipir_dbmul")
+
+
+def dbmul_host(plan, d_db, h_query, h_answer, stream=None):
+    """vipir_dbmul_host: host query in, host answer out; synchronises the stream."""
+    _check(load().vipir_dbmul_host(plan, _ptr(d_db), _ptr(h_query), _ptr(h_answer), _stream_ptr(stream)),
+           "vipir_dbmul_host")
+
+
+def split_limbs(plan, d_query, d_planes_out=None, stream=None):
+    """vipir_split_limbs: step a1 alone, into d_planes_out (or the plan's workspace if None)."""
+    out = ctypes.c_void_p(None) if d_planes_out is None else _ptr(d_planes_out)
+    _check(load().vipir_split_limbs(plan, _ptr(d_query), out, _stream_ptr(stream)), "vipir_split_limbs")
+
+
+def plan_info(plan) -> dict:
+    info = Info()
+    _check(load().vipir_plan_info(plan, ctypes.byref(info)), "vipir_plan_info")
+    return info.as_dict()
+
+
+def destroy(plan):
+    load().vipir_destroy(plan)
+
+
+class Plan:
+    """Context-manager convenience around dbmul_plan / destroy."""
+
+    def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO):
+        self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime)
+        self.info = plan_info(self.handle)
+
+    def __call__(self, d_db, d_query, d_answer, stream=None):
+        dbmul(self.handle, d_db, d_query, d_answer, stream)
+
+    def host(self, d_db, h_query, h_answer, stream=None):
+        dbmul_host(self.handle, d_db, h_query, h_answer, stream)
+
+    def close(self):
+        if self.handle is not None:
+            destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,106 @@
+"""Host-side checks of the C ABI that need no GPU: the library loads, exports every symbol
+include/vipir.h declares, and rejects bad arguments before touching CUDA."""
+import ctypes
+import re
+from pathlib import Path
+
+import pytest
+
+from paper_2606_11536_b200 import build, vipir
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return vipir.load()
+
+
+def test_header_symbols_are_exported(lib):
+    header = (ROOT / "include" / "vipir.h").read_text()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)  # declarations only, not comments
+    declared = set(re.findall(r"\b(vipir_[a-z_]+)\s*\(", header))
+    assert declared == set(vipir.SYMBOLS), declared ^ set(vipir.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_status_strings(lib):
+    names = [lib.vipir_status_str(i).decode() for i in range(6)]
+    assert names == ["VIPIR_OK", "VIPIR_ERR_INVALID_ARG", "VIPIR_ERR_UNSUPPORTED", "VIPIR_ERR_ALLOC",
+                     "VIPIR_ERR_CUDA", "VIPIR_ERR_ARCH"]
+    assert lib.vipir_status_str(99).decode() == "VIPIR_ERR_UNKNOWN"
+
+
+def test_destroy_null_is_noop(lib):
+    lib.vipir_destroy(None)
+
+
+def _plan_status(lib, rows, cols, batch, db_bits, moduli=None, regime=0, count=None):
+    h = ctypes.c_void_p()
+    spec_p = None
+    if moduli is not None or count is not None:
+        arr = (ctypes.c_uint32 * max(1, len(moduli or [])))(*(moduli or [0]))
+        spec = vipir.ModulusSpec(len(moduli) if count is None else count, arr if moduli is not None else None)
+        spec_p = ctypes.byref(spec)
+    st = lib.vipir_dbmul_plan_ex(ctypes.byref(h), rows, cols, batch, db_bits, spec_p, regime)
+    assert st != vipir.OK or h.value
+    if st == vipir.OK:
+        lib.vipir_destroy(h)
+    return st
+
+
+@pytest.mark.parametrize("args", [
+    dict(rows=0, cols=16, batch=1, db_bits=8),
+    dict(rows=16, cols=0, batch=1, db_bits=8),
+    dict(rows=16, cols=16, batch=0, db_bits=8),
+    dict(rows=16, cols=16, batch=1, db_bits=12),
+    dict(rows=16, cols=16, batch=1, db_bits=8, moduli=[1]),
+    dict(rows=16, cols=16, batch=1, db_bits=8, moduli=[1 << 30]),
+    dict(rows=16, cols=16, batch=1, db_bits=8, moduli=[97, 101, 103, 107, 109]),
+    dict(rows=16, cols=16, batch=1, db_bits=8, count=2),  # count > 0 with a null moduli pointer
+    dict(rows=16, cols=16, batch=1, db_bits=8, regime=9),
+])
+def test_invalid_arguments(lib, args):
+    assert _plan_status(lib, **args) == vipir.ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("args", [
+    dict(rows=16, cols=24, batch=1, db_bits=8),        # row bytes not a multiple of 16
+    dict(rows=16, cols=4, batch=1, db_bits=16),
+    dict(rows=1 << 31, cols=16, batch=1, db_bits=8),   # beyond the stated size limit
+    dict(rows=16, cols=1 << 31, batch=1, db_bits=8),
+])
+def test_unsupported_shapes(lib, args):
+    assert _plan_status(lib, **args) == vipir.ERR_UNSUPPORTED
+
+
+def test_null_out_pointer(lib):
+    assert lib.vipir_dbmul_plan_ex(None, 16, 16, 1, 8, None, 0) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_dbmul(None, None, None, None, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_dbmul_host(None, None, None, None, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_plan_info(None, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_split_limbs(None, None, None, None) == vipir.ERR_INVALID_ARG
+
+
+def test_no_silent_fallback_without_a_gpu(lib):
+    """On a box without a B200 a valid plan request must fail loudly (CUDA/ARCH), never succeed."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    st = _plan_status(lib, 1024, 1024, 1, 8)
+    assert st in (vipir.ERR_CUDA, vipir.ERR_ARCH)
+    with pytest.raises(vipir.VipirError):
+        vipir.dbmul_plan(1024, 1024, 1)
+
+
+def test_product_never_imports_the_oracle():
+    pkg = ROOT / "paper_2606_11536_b200"
+    for f in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.cuh")) + [ROOT / "include" / "vipir.h"]:
+        text = f.read_text()
+        assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), f
+        assert "vipir_oracle" not in text, f
+    for f in (ROOT / "oracle").rglob("*.py"):
+        assert not re.search(r"^\s*(from|import)\s+paper_2606_11536_b200\b", f.read_text(), re.M), f
+    assert "#include \"" not in (ROOT / "oracle" / "vipir_oracle.c").read_text()  # system headers only

@@ -1,0 +1,263 @@
+"""GPU parity: libvipir (through the C ABI) against the CPU oracle, bit for bit.
+
+All work is integer, so the bar is exact equality of every compared word (no tolerance).
+Small and medium shapes are compared in full and are sized to span several tiles plus a
+ragged tail in every dimension (rows, K bytes, query vectors, K chunks); BASELINE.json's
+full-size configs are compared on sampled rows the oracle computes one by one, plus a
+column-sum identity that covers every row at any size (tests/test_parity_fullsize_gpu.py).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_11536_b200 import inputs, vipir
+
+from gpu_util import ensure_built, run_dbmul
+
+pytestmark = pytest.mark.gpu
+
+PRIMES = inputs.rns_primes(0)
+NT = max(1, os.cpu_count() or 1)
+G, M1, M2, NAIVE, AUTO = (vipir.REGIME_GEMV, vipir.REGIME_MMA_1SM, vipir.REGIME_MMA_2SM, vipir.REGIME_NAIVE,
+                          vipir.REGIME_AUTO)
+
+
+def make(seed, rows, cols, batch, db_bits=8, moduli=None):
+    return inputs.db_rows(seed, rows, cols, db_bits), inputs.query(seed, cols, batch, moduli)
+
+
+def assert_same(got, want):
+    bad = np.argwhere(got != want)
+    assert bad.size == 0, (f"{len(bad)} of {got.size} words differ; first at [t,b,r]={bad[0].tolist()}: "
+                           f"got {got[tuple(bad[0])]} want {want[tuple(bad[0])]}")
+
+
+def check(D, Q, moduli, regime):
+    got = run_dbmul(D, Q, moduli, regime)
+    want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+    assert_same(got, want)
+
+
+# ---- a1: the limb splitter on its own --------------------------------------
+
+@pytest.mark.parametrize("db_bits,moduli,cols,batch", [
+    (8, None, 1040, 3), (16, None, 520, 2), (16, PRIMES, 264, 2), (8, None, 16, 1), (8, PRIMES, 48, 1)])
+def test_split_limbs_planes(db_bits, moduli, cols, batch):
+    import torch
+    ensure_built()
+    Q = inputs.query(31, cols, batch, moduli)
+    Q[0, 0, :3] = [0xFFFFFFFF, 0x01020304, 0x80000000]
+    d_q = torch.from_numpy(Q.view(np.int32)).cuda()
+    dl = db_bits // 8
+    with vipir.Plan(256, cols, batch, db_bits, moduli, M1) as plan:
+        lc, nq, kb = plan.info["limb_cols"], plan.info["query_vectors"], plan.info["k_bytes"]
+        assert lc == (5 if (dl == 2 and moduli) else 4) and nq == Q.shape[0] * batch and kb == cols * dl
+        assert plan.info["workspace_bytes"] == nq * lc * kb
+        planes = torch.full((nq * lc * kb,), 0xAA, dtype=torch.uint8, device="cuda")
+        vipir.split_limbs(plan.handle, d_q, planes)
+        torch.cuda.synchronize()
+    got = planes.cpu().numpy().reshape(nq, lc, kb)
+    Qf = Q.reshape(nq, cols)
+    limb = [((Qf >> (8 * j)) & 0xFF).astype(np.uint8) for j in range(4)]  # B_j of PAPER.md:245
+    for s in range(lc):
+        if dl == 1:
+            want = limb[s]
+        else:
+            want = np.zeros((nq, kb), dtype=np.uint8)
+            if s < 4:
+                want[:, 0::2] = limb[s]
+            if s >= 1:
+                want[:, 1::2] = limb[s - 1]
+        assert np.array_equal(got[:, s, :], want), f"plane s={s}"
+
+
+# ---- test-only check kernel ---------------------------------------------------------------------
+
+@pytest.mark.parametrize("db_bits,moduli", [(8, None), (16, None), (8, PRIMES), (16, PRIMES)])
+def test_naive_kernel(db_bits, moduli):
+    D, Q = make(41, 70, 48 // (db_bits // 8) * 4, 3, db_bits, moduli)
+    check(D, Q, moduli, NAIVE)
+
+
+# ---- a2: batch-1 scan (GEMV regime) ------------------------------------------------------------
+
+@pytest.mark.parametrize("rows,cols", [(1024, 1024), (100, 4112), (33, 16), (1, 16), (257, 2064), (32, 1024), (64, 3072)])
+def test_gemv_u8(rows, cols):
+    D, Q = make(rows + cols, rows, cols, 1)
+    check(D, Q, None, G)
+
+
+def test_gemv_u16_wrapping():
+    D, Q = make(43, 70, 520, 1, 16)
+    check(D, Q, None, G)
+
+
+def test_gemv_extremes_and_permutation():
+    rows, cols = 96, 2048
+    D = np.full((rows, cols), 255, dtype=np.uint8)
+    Q = np.full((1, 1, cols), 0xFFFFFFFF, dtype=np.uint32)
+    got = run_dbmul(D, Q, None, G)
+    assert (got == (-255 * cols) % (1 << 32)).all()  # closed form 2 of SURVEY.md 8(c)
+    perm = np.random.default_rng(1).integers(0, cols, size=rows)
+    D = np.zeros((rows, cols), dtype=np.uint8)
+    D[np.arange(rows), perm] = 1
+    Q = (np.arange(cols, dtype=np.uint32) + 1).reshape(1, 1, cols)
+    assert np.array_equal(run_dbmul(D, Q, None, G)[0, 0], (perm + 1).astype(np.uint32))
+
+
+# ---- a3/a4: tensor-core regimes, q = 2^32 --------------------------------------------------------
+
+@pytest.mark.parametrize("regime", [M1, M2])
+@pytest.mark.parametrize("batch", [1, 2, 3, 8, 16, 64, 100])
+def test_mma_u8_wrapping(regime, batch):
+    # rows: 2 full M tiles + ragged tail (44 rows); K: 12 k-steps + 16-byte tail
+    D, Q = make(100 + batch, 300, 1552, batch)
+    check(D, Q, None, regime)
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_permutation_probe(regime):
+    # catches swizzle / descriptor / layout errors as permuted results
+    rows, cols, batch = 256, 512, 8
+    rng = np.random.default_rng(2)
+    perm = rng.integers(0, cols, size=rows)
+    D = np.zeros((rows, cols), dtype=np.uint8)
+    D[np.arange(rows), perm] = 1
+    Q = np.stack([(np.arange(cols, dtype=np.uint64) + 1) * (b + 1) * 0x01010101 % (1 << 32) for b in range(batch)])
+    Q = Q.astype(np.uint32).reshape(1, batch, cols)
+    got = run_dbmul(D, Q, None, regime)
+    for b in range(batch):
+        assert np.array_equal(got[0, b], Q[0, b, perm]), f"query {b}"
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_large_batch_two_n_tiles(regime):
+    D, Q = make(51, 260, 1040, 256)
+    got, info = run_dbmul(D, Q, None, regime, return_info=True)
+    assert info["n_tiles"] >= 2
+    assert_same(got, oracle.dbmul(D, Q, None, nthreads=NT))
+
+
+# ---- K chunking: int32 accumulators at their limit (R7) ------------------------------
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_chunk_seams_adversarial(regime, golden):
+    cols = 32768 * 2 + 4112  # three chunks, ragged
+    rows, batch = 130, 2
+    D = np.full((rows, cols), 255, dtype=np.uint8)
+    Q = np.full((1, batch, cols), 0xFFFFFFFF, dtype=np.uint32)
+    got, info = run_dbmul(D, Q, None, regime, return_info=True)
+    assert info["n_chunks"] == 3 and info["k_chunk_bytes"] <= golden["int32_chunk_bound"]["k_chunk_contract"]
+    assert (got == (-255 * cols) % (1 << 32)).all()
+    D, Q = make(52, rows, cols, batch)
+    D[:64] = 255
+    check(D, Q, None, regime)
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_exact_chunk_of_32768_all_max(regime):
+    cols = 32768
+    D = np.full((128, cols), 255, dtype=np.uint8)
+    Q = np.full((1, 4, cols), 0xFFFFFFFF, dtype=np.uint32)
+    got = run_dbmul(D, Q, None, regime)
+    assert (got == (-255 * cols) % (1 << 32)).all()
+    p = PRIMES[0]
+    got = run_dbmul(D, Q, [p], regime)  # true integer sums needed: no wrap may hide an overflow
+    assert (got == (255 * 0xFFFFFFFF * cols) % p).all()
+
+
+# ---- a4/a5: prime moduli, u16 DB -------------------------------------------------------------------
+
+@pytest.mark.parametrize("regime", [M1, M2])
+@pytest.mark.parametrize("db_bits,moduli,batch", [
+    (8, PRIMES, 5), (8, [PRIMES[0]], 1), (16, None, 4), (16, PRIMES, 3), (16, PRIMES, 40), (16, [97, 1 << 29, 2, PRIMES[1]], 2)])
+def test_mma_moduli_and_u16(regime, db_bits, moduli, batch):
+    D, Q = make(60 + batch, 300, 776 if db_bits == 16 else 1552, batch, db_bits, moduli)
+    check(D, Q, moduli, regime)
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_prime_edges(regime):
+    p = PRIMES[0]
+    cols = 40000
+    D = np.ones((130, cols), dtype=np.uint16)
+    Q = np.full((1, 2, cols), p - 1, dtype=np.uint32)
+    got = run_dbmul(D, Q, [p], regime)
+    assert (got == (-cols) % p).all()  # closed form 3
+    D = np.full((130, cols), 0xFFFF, dtype=np.uint16)
+    Q = np.full((2, 1, cols), 0xFFFFFFFF, dtype=np.uint32)  # words above the modulus are legal (R5)
+    got = run_dbmul(D, Q, PRIMES, regime)
+    for t, pt in enumerate(PRIMES):
+        assert (got[t] == (0xFFFF * 0xFFFFFFFF * cols) % pt).all()
+        assert (got[t] < pt).all()
+
+
+# ---- planner / ABI behaviour on the device ------------------------------------------------------
+
+def test_auto_regime_choice():
+    ensure_built()
+    with vipir.Plan(1024, 1024, 1) as p:
+        assert p.info["regime_name"] == "gemv" and p.info["launches"] == 2
+    with vipir.Plan(1024, 1024, 8) as p:
+        assert p.info["regime_name"] == "mma_1sm" and p.info["mma_n"] == 32
+    with vipir.Plan(1024, 1024, 256) as p:
+        assert p.info["regime_name"] == "mma_2sm" and p.info["tile_cols"] == 512 and p.info["n_tiles"] == 2
+    with vipir.Plan(1024, 1024, 1, 8, [PRIMES[0]]) as p:
+        assert p.info["regime_name"] == "mma_1sm"
+    with vipir.Plan(32768, 32768, 64, 16, PRIMES) as p:
+        assert p.info["limb_cols"] == 5 and p.info["k_bytes"] == 65536 and p.info["n_chunks"] == 2
+    with pytest.raises(vipir.VipirError) as e:
+        vipir.Plan(1024, 1024, 2, regime=G)
+    assert e.value.status == vipir.ERR_UNSUPPORTED
+
+
+def test_auto_matches_oracle_on_config_1():
+    # BASELINE.json configs[0]: D 1024x1024 u8, Q 1024x1 u32, q = 2^32, seed 0
+    D, Q = make(0, 1024, 1024, 1)
+    check(D, Q, None, AUTO)
+
+
+def test_plan_reuse_with_new_buffers_and_host_entry_point():
+    import torch
+    ensure_built()
+    rows, cols, batch = 200, 1040, 8
+    with vipir.Plan(rows, cols, batch) as plan:
+        for seed in (70, 71):
+            D, Q = make(seed, rows, cols, batch)
+            d_db = torch.from_numpy(D).cuda()
+            d_q = torch.from_numpy(Q.view(np.int32)).cuda()
+            d_a = torch.empty((1, batch, rows), dtype=torch.int32, device="cuda")
+            plan(d_db, d_q, d_a)
+            torch.cuda.synchronize()
+            assert_same(d_a.cpu().numpy().view(np.uint32), oracle.dbmul(D, Q))
+        h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+        h_a = torch.empty((1, batch, rows), dtype=torch.int32).pin_memory()
+        plan.host(d_db, h_q, h_a)
+        assert_same(h_a.numpy().view(np.uint32), oracle.dbmul(D, Q))
+
+
+def test_misaligned_pointers_are_rejected():
+    import torch
+    ensure_built()
+    with vipir.Plan(64, 64, 1) as plan:
+        buf = torch.zeros(64 * 64 + 64, dtype=torch.uint8, device="cuda")
+        q = torch.zeros(64, dtype=torch.int32, device="cuda")
+        a = torch.zeros(64, dtype=torch.int32, device="cuda")
+        with pytest.raises(vipir.VipirError) as e:
+            vipir.dbmul(plan.handle, buf.data_ptr() + 1, q, a)
+        assert e.value.status == vipir.ERR_INVALID_ARG
+
+
+def test_toy_lwe_roundtrip_through_the_gpu():
+    """SimplePIR end to end: the GPU's answer decrypts to the
+    selected DB column.  Uses the oracle package's toy client only for keys/queries/decrypt."""
+    from oracle import lwe
+    cols, rows, n = 1024, 200, 15  # n+1 = 16 query vectors
+    g = np.random.default_rng(5)
+    D = inputs.db_rows(77, rows, cols, 8)
+    s = lwe.keygen(n, g)
+    Q, _ = lwe.simplepir_query(cols, 321, s, g)
+    A = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO)[0]
+    assert np.array_equal(lwe.decrypt_answer(A, s), D[:, 321])
