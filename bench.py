@@ -1,0 +1,388 @@
+#!/usr/bin/env python
+"""bench.py -- the VIPIR database scan on B200, measured.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--all]
+
+Headline (BASELINE.json `metric`: "DB GB/s scanned & TOPS, % of HBM/INT8-TC roofline; 16 GiB u8
+DB, batch 1/256"): one STEP is one pass of the whole hot path -- query-limb splitter + scan
+kernel, through the C ABI (vipir_dbmul) -- over one batch of synthetic queries against the
+16 GiB u8 database of configs[2] (131072 x 131072, q = 2^32, batch 1).  `value` is GB of DB
+scanned per second with all inputs resident in HBM; `e2e` is the same through vipir_dbmul_host
+with the query in / the answer out of pinned HOST memory inside the timed region.  The batched
+tensor-core regime (configs[3], 4 GiB, batch 256) and the other configs are measured in the
+same run and reported under "batched" / "configs" of the same JSON line.
+
+The DB (16 GiB) is far larger than the 126 MB L2, so no L2 flush is needed between steps.
+N > 1 (torchrun): the path shards by DB rows with no data-path collective (each
+GPU holds a (D1/#GPU) x D0 partition; queries are broadcast) -- every rank scans its own
+16 GiB row shard (weak scaling); value = all ranks' bytes / max-over-ranks device time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on this box's host cores on a
+bounded row sample of the same workload and prints the same JSON line with "impl": "reference".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "db_scan_GBps_16GiB_u8_batch1"
+UNIT = "GB/s"
+SEED = 0
+
+# BASELINE.json configs (rows, cols, batch, db_bits, prime moduli?)
+CONFIGS = {
+    "C1_tiny_B1": (1024, 1024, 1, 8, False),
+    "C2_1GiB_B1": (32768, 32768, 1, 8, False),
+    "C3_16GiB_B1": (131072, 131072, 1, 8, False),
+    "C3_16GiB_B8": (131072, 131072, 8, 8, False),
+    "C4_4GiB_B256": (65536, 65536, 256, 8, False),
+    "C5_rns_u16_B64x2": (32768, 32768, 64, 16, True),
+}
+HEADLINE = "C3_16GiB_B1"
+BATCHED = "C4_4GiB_B256"
+
+
+# ---- host-side helpers (also exercised by the gloo tests) -------------------------------------
+
+def shard_rows(rank: int, world: int, rows_per_gpu: int):
+    """Weak scaling over DB rows: rank r owns global rows [r*rows_per_gpu, (r+1)*rows_per_gpu)
+    of a (world*rows_per_gpu) x cols database (row sharding)."""
+    return rank * rows_per_gpu, (rank + 1) * rows_per_gpu
+
+
+def aggregate(per_rank_ms, units_per_rank: float, steps: int):
+    """Whole-job throughput: all ranks' units / the slowest rank's device time."""
+    t_ms = max(per_rank_ms)
+    total_units = units_per_rank * len(per_rank_ms) * steps
+    return total_units / (t_ms * 1e-3), t_ms / steps
+
+
+def measured_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        d = json.loads(f.read_text())
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_burst": float(d["bf16_tflops"]),
+                "bf16_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "source": "measured"}
+    # fallback stated in B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+def profiled_traffic(kernel: str):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
+    f = ROOT / "profiles" / "traffic.json"
+    if f.exists():
+        return json.loads(f.read_text()).get(kernel)
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self.index, self.period = index, period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    _NAMES = {
+        0x0000000000000004: "sw_power_cap", 0x0000000000000008: "hw_slowdown",
+        0x0000000000000020: "sw_thermal_slowdown", 0x0000000000000040: "hw_thermal_slowdown",
+        0x0000000000000080: "hw_power_brake_slowdown", 0x0000000000000002: "applications_clocks_setting",
+        0x0000000000000010: "sync_boost", 0x0000000000000100: "display_clocks_setting",
+    }
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                r = self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in self._NAMES.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ---- the CUDA arm ---------------------------------------------------------------------------
+
+def time_events(fn, steps, warmup, stream):
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)  # ms for `steps` calls
+
+
+def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset_bytes=0):
+    """Times one config on the current device; returns a dict of measurements."""
+    import torch
+    from paper_2606_11536_b200 import inputs, vipir
+    from paper_2606_11536_b200.inputs import device
+    rows, cols, batch, db_bits, prime = CONFIGS[name]
+    moduli = inputs.rns_primes(SEED) if prime else None
+    kb = cols * db_bits // 8
+    d_db = device_db[row_offset_bytes: row_offset_bytes + rows * kb].view(rows, kb)
+    d_q = device.query(SEED, cols, batch, moduli)
+    T = d_q.shape[0]
+    d_a = torch.empty((T, batch, rows), dtype=torch.int32, device="cuda")
+    stream = torch.cuda.current_stream()
+    out = {"rows": rows, "cols": cols, "batch": batch, "db_bits": db_bits, "moduli": moduli or "2^32"}
+    with vipir.Plan(rows, cols, batch, db_bits, moduli) as plan:
+        info = plan.info
+        ms_step = time_events(lambda: plan(d_db, d_q, d_a), steps, warmup, stream) / steps
+        # the dominant kernel alone (planes already in the workspace) and the splitter alone
+        ms_scan = time_events(lambda: vipir.dbmul_scan(plan.handle, d_db, d_a), steps, warmup, stream) / steps
+        ms_split = time_events(lambda: vipir.split_limbs(plan.handle, d_q), steps, warmup, stream) / steps
+        if with_e2e:
+            h_q = d_q.cpu().pin_memory()
+            h_a = torch.empty((T, batch, rows), dtype=torch.int32).pin_memory()
+            for _ in range(warmup):
+                plan.host(d_db, h_q, h_a)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(steps):
+                plan.host(d_db, h_q, h_a)  # H2D query, split, scan, D2H answer, stream sync -- every step
+            e1.record(stream)
+            torch.cuda.synchronize()
+            out["e2e_ms"] = e0.elapsed_time(e1) / steps
+            out["h2d_bytes"] = h_q.numel() * 4
+            out["d2h_bytes"] = h_a.numel() * 4
+    db_bytes = rows * kb
+    nq, lc = info["query_vectors"], info["limb_cols"]
+    logical_ops = 2.0 * rows * cols * nq
+    int8_ops = 2.0 * rows * kb * nq * lc  # what the tensor pipe executes (limb MACs)
+    alg_bytes = db_bytes + 4 * cols * nq + 4 * rows * nq  # DB + query + answer
+    out.update({
+        "regime": info["regime_name"], "ms_per_step": ms_step, "ms_scan_kernel": ms_scan, "ms_split_kernel": ms_split,
+        "db_GBps": db_bytes / ms_step / 1e6, "scan_kernel_GBps": alg_bytes / ms_scan / 1e6,
+        "logical_TOPS": logical_ops / ms_step / 1e9, "int8_TOPS": int8_ops / ms_step / 1e9,
+        "scan_kernel_int8_TOPS": int8_ops / ms_scan / 1e9,
+        "frac_hbm_measured": alg_bytes / ms_scan / 1e6 / peaks["hbm_gbs"],
+        "frac_hbm_nominal_8TBps": db_bytes / ms_step / 1e6 / 8000.0,
+        "frac_int8_nominal_4500": int8_ops / ms_step / 1e9 / 4500.0,
+        "frac_int8_measured_sustained": int8_ops / ms_scan / 1e9 / (2.0 * peaks["bf16_sustained"]),
+        "plan": {k: info[k] for k in ("tile_cols", "mma_n", "m_tiles", "n_tiles", "n_chunks", "k_chunk_bytes", "stages",
+                                       "grid", "smem_bytes", "launches")},
+        "alg_bytes": alg_bytes, "int8_ops": int8_ops,
+    })
+    del d_q, d_a
+    return out
+
+
+def cpu_baseline(sample_rows: int, device_db, cols: int):
+    """The oracle, as it stands, on the host cores, on the first `sample_rows` rows of the
+    headline workload (same bytes: copied back from the device-generated DB)."""
+    import numpy as np
+    import oracle
+    from paper_2606_11536_b200 import inputs
+    D = device_db[: sample_rows * cols].view(sample_rows, cols).cpu().numpy()
+    Q = inputs.query(SEED, cols, 1)
+    cores = os.cpu_count() or 1
+    oracle.dbmul(D[:64], Q, nthreads=cores)  # load + warm
+    t0 = time.perf_counter()
+    A = oracle.dbmul(D, Q, nthreads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": D.size / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {sample_rows} of 131072 rows x 131072 cols, batch 1 ({D.size / 2**30:.0f} GiB of DB), "
+                      f"{dt:.2f} s wall on {cores} threads", "seconds": dt}, A
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_11536_b200 import build, vipir
+    from paper_2606_11536_b200.inputs import device, generator
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    build.build()
+    vipir.load()
+    peaks = measured_peaks()
+
+    rows, cols, _, _, _ = CONFIGS[HEADLINE]
+    # this rank's row shard of the (world*rows) x cols DB: same stream, offset by the shard's first byte
+    r0, _ = shard_rows(rank, world, rows)
+    nbytes = rows * cols
+    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    lib = device._load()
+    import ctypes
+    key = generator.stream_key(SEED + 1000003 * rank, generator.STREAM_DB) if world > 1 else generator.stream_key(SEED, generator.STREAM_DB)
+    rc = lib.vipir_inputs_fill_bytes(buf.data_ptr(), nbytes, key, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert rc == 0
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- headline: timed region bracketed by barrier + synchronize, clocks sampled during it ----
+    barrier()
+    with ClockSampler(local_rank) as clk:
+        head = run_config(HEADLINE, buf, args.steps, args.warmup, peaks, with_e2e=True)
+    barrier()
+    times = [head["ms_per_step"] * args.steps]
+    e2e_times = [head["e2e_ms"] * args.steps]
+    if world > 1:
+        t = torch.tensor([times[0], e2e_times[0]], dtype=torch.float64, device="cuda")
+        gathered = [torch.zeros_like(t) for _ in range(world)]
+        dist.all_gather(gathered, t)
+        times = [float(g[0]) for g in gathered]
+        e2e_times = [float(g[1]) for g in gathered]
+    value, ms_per_step = aggregate(times, nbytes / 1e9, args.steps)
+    e2e_value, _ = aggregate(e2e_times, nbytes / 1e9, args.steps)
+
+    extra = {}
+    cpu = None
+    if rank == 0 and world == 1:
+        steps2 = max(3, min(args.steps, 20))
+        for name in ([BATCHED] if not args.all else [n for n in CONFIGS if n != HEADLINE]):
+            extra[name] = run_config(name, buf, steps2, max(3, min(args.warmup, 5)), peaks)
+        cpu, _ = cpu_baseline(args.cpu_sample_rows, buf, cols)
+
+    if rank == 0:
+        b = extra.get(BATCHED)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8*u32->u32 (mod 2^32)", "data": "synthetic",
+            "config": {"workload": "configs[2]: 16 GiB u8 DB 131072x131072 uniform, Q 131072x1 u32 uniform, q=2^32, "
+                                   "seed 0; per GPU (row-sharded for N>1)",
+                       "regime": head["regime"], "l2": "inputs (16 GiB) larger than L2; no flush",
+                       "plan": head["plan"]},
+            "clocks": clk.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": head["h2d_bytes"],
+                    "d2h_bytes_per_step": head["d2h_bytes"], "ms_per_step": head["e2e_ms"]},
+            "gpu_launches": head["plan"]["launches"] * args.steps,
+            "roofline": {"bound": "hbm", "kernel": "gemv_b1_kernel", "achieved": head["scan_kernel_GBps"],
+                         "peak": peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)"
+                         if peaks["source"] == "measured" else "fallback 6650 GB/s (B200_PROFILING.md)",
+                         "unit": "GB/s", "frac": head["frac_hbm_measured"],
+                         "frac_of_nominal_8TBps": head["scan_kernel_GBps"] / 8000.0,
+                         "ms_per_launch": head["ms_scan_kernel"], "alg_bytes_per_launch": head["alg_bytes"],
+                         "traffic": profiled_traffic("gemv_b1_kernel")},
+            "cpu_baseline": cpu,
+        }
+        if b:
+            line["batched"] = {
+                "workload": "configs[3]: 4 GiB u8 DB 65536x65536, Q 65536x256 u32, q=2^32, 4 int8 limbs, K chunks <= 32768",
+                "ms_per_step": b["ms_per_step"], "db_GBps": b["db_GBps"], "logical_TOPS": b["logical_TOPS"],
+                "int8_TOPS": b["int8_TOPS"], "regime": b["regime"], "plan": b["plan"],
+                "roofline": {"bound": "tensor", "kernel": "gemm_i8_kernel<2,4,false>", "achieved": b["scan_kernel_int8_TOPS"],
+                             "peak": 2.0 * peaks["bf16_sustained"], "unit": "TOP/s (int8)",
+                             "peak_source": "2 x measured sustained bf16 (nominal int8:bf16 = 4.5:2.25)",
+                             "frac": b["frac_int8_measured_sustained"],
+                             "frac_of_nominal_4500": b["scan_kernel_int8_TOPS"] / 4500.0,
+                             "ms_per_launch": b["ms_scan_kernel"], "int8_ops_per_launch": b["int8_ops"],
+                             "traffic": profiled_traffic("gemm_i8_kernel")},
+            }
+        if args.all:
+            line["configs"] = {n: {k: v for k, v in r.items() if k not in ("alg_bytes", "int8_ops")} for n, r in extra.items()}
+            line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in ("alg_bytes", "int8_ops")}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ---- the reference arm: the oracle on the host cores ---------------------------------------
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import oracle
+    from paper_2606_11536_b200 import inputs
+    rows, cols, _, _, _ = CONFIGS[HEADLINE]
+    sample = args.ref_sample_rows
+    cores = os.cpu_count() or 1
+    oracle.build()
+    D = inputs.db_rows(SEED, rows, cols, 8, 0, sample)
+    Q = inputs.query(SEED, cols, 1)
+    for _ in range(args.warmup):
+        oracle.dbmul(D, Q, nthreads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.dbmul(D, Q, nthreads=cores)
+    dt = time.perf_counter() - t0
+    value = D.size * args.steps / dt / 1e9
+    desc = f"each step = first {sample} of 131072 rows x 131072 cols, batch 1 ({D.size / 2**20:.0f} MiB of DB)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8*u32->u128 accumulate, % 2^32", "data": "synthetic",
+        "config": {"workload": "configs[2] (16 GiB u8 DB, batch 1), bounded row sample: " + desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--all", action="store_true", help="also time every other BASELINE.json config")
+    ap.add_argument("--cpu-sample-rows", type=int, default=32768)
+    ap.add_argument("--ref-sample-rows", type=int, default=4096)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

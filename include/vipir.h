@@ -136,6 +136,11 @@ int vipir_dbmul_host(vipir_plan *plan, const void *d_db, const uint32_t *h_query
  * (DEVICE, 16-byte aligned, workspace_bytes long), or into the plan's workspace if NULL. */
 int vipir_split_limbs(vipir_plan *plan, const uint32_t *d_query, uint8_t *d_planes_out, void *cuda_stream);
 
+/* Run only the scan kernel (steps a2 or a3+a4) against the limb planes already in the plan's
+ * workspace (written by the last vipir_dbmul or vipir_split_limbs(plan, q, NULL, ...) call).
+ * vipir_dbmul == vipir_split_limbs + vipir_dbmul_scan.  For per-kernel timing and tests. */
+int vipir_dbmul_scan(vipir_plan *plan, const void *d_db, uint32_t *d_answer, void *cuda_stream);
+
 /* Describe the plan.  Errors: INVALID_ARG. */
 int vipir_plan_info(const vipir_plan *plan, vipir_info *out);
 

@@ -333,6 +333,32 @@ int vipir_split_limbs(vipir_plan* p, const uint32_t* d_query, uint8_t* d_planes_
     return launch_split(p, d_query, d_planes_out ? d_planes_out : p->d_planes, static_cast<cudaStream_t>(cuda_stream));
 }
 
+static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaStream_t st) {
+    int rc = encode_db_map(p, d_db);
+    if (rc != VIPIR_OK) return rc;
+    if (p->regime == VIPIR_REGIME_GEMV) {
+        static thread_local bool attr_set = false;
+        if (!attr_set) {
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+            attr_set = true;
+        }
+        p->gv.answer = d_answer;
+        vipir::gemv_b1_kernel<<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        CK(cudaGetLastError());
+        return VIPIR_OK;
+    }
+    p->gm.answer = d_answer;
+    return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
+}
+
+int vipir_dbmul_scan(vipir_plan* p, const void* d_db, uint32_t* d_answer, void* cuda_stream) {
+    if (!p || !d_db || !d_answer) return VIPIR_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_answer) & 3))
+        return VIPIR_ERR_INVALID_ARG;
+    if (p->regime == VIPIR_REGIME_NAIVE) return VIPIR_ERR_UNSUPPORTED;  // the check kernel has no limb planes
+    return scan_only(p, d_db, d_answer, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32_t* d_answer, void* cuda_stream) {
     if (!p || !d_db || !d_query || !d_answer) return VIPIR_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
@@ -352,25 +378,9 @@ int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
-
-    int rc = encode_db_map(p, d_db);
+    int rc = launch_split(p, d_query, p->d_planes, st);
     if (rc != VIPIR_OK) return rc;
-    rc = launch_split(p, d_query, p->d_planes, st);
-    if (rc != VIPIR_OK) return rc;
-
-    if (p->regime == VIPIR_REGIME_GEMV) {
-        static thread_local bool attr_set = false;
-        if (!attr_set) {
-            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-            attr_set = true;
-        }
-        p->gv.answer = d_answer;
-        vipir::gemv_b1_kernel<<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
-        CK(cudaGetLastError());
-        return VIPIR_OK;
-    }
-    p->gm.answer = d_answer;
-    return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
+    return scan_only(p, d_db, d_answer, st);
 }
 
 int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, uint32_t* h_answer, void* cuda_stream) {

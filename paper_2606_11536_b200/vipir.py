@@ -23,7 +23,7 @@ MAX_MODULI = 4
 
 # every symbol include/vipir.h declares
 SYMBOLS = (
-    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs",
+    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
 )
 
@@ -82,6 +82,8 @@ def load() -> ctypes.CDLL:
         lib.vipir_dbmul_host.argtypes = [vp, vp, vp, vp, vp]
         lib.vipir_split_limbs.restype = i
         lib.vipir_split_limbs.argtypes = [vp, vp, vp, vp]
+        lib.vipir_dbmul_scan.restype = i
+        lib.vipir_dbmul_scan.argtypes = [vp, vp, vp, vp]
         lib.vipir_plan_info.restype = i
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
@@ -145,6 +147,11 @@ def split_limbs(plan, d_query, d_planes_out=None, stream=None):
     """vipir_split_limbs: step a1 alone, into d_planes_out (or the plan's workspace if None)."""
     out = ctypes.c_void_p(None) if d_planes_out is None else _ptr(d_planes_out)
     _check(load().vipir_split_limbs(plan, _ptr(d_query), out, _stream_ptr(stream)), "vipir_split_limbs")
+
+
+def dbmul_scan(plan, d_db, d_answer, stream=None):
+    """vipir_dbmul_scan: the scan kernel alone, against the planes already in the workspace."""
+    _check(load().vipir_dbmul_scan(plan, _ptr(d_db), _ptr(d_answer), _stream_ptr(stream)), "vipir_dbmul_scan")
 
 
 def plan_info(plan) -> dict:
