@@ -64,7 +64,7 @@ typedef struct {
 } vipir_modulus_spec;
 
 /* Kernel regimes.  AUTO picks GEMV for one wrapping query vector,
- * otherwise the tensor-core path (1-SM tiles while the product is HBM-bound, 2-SM pairs
+ * otherwise the tensor-core path (1-SM tiles up to 16 query vectors, 2-SM pairs
  * above).  NAIVE is a test-only check kernel and is never picked by AUTO. */
 typedef enum {
     VIPIR_REGIME_AUTO = 0,

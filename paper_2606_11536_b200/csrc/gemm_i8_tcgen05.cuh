@@ -48,11 +48,13 @@ struct GemmParams {
     uint32_t n_tiles, m_tiles;
     uint32_t ni_cols;        // N of one MMA instruction
     uint32_t n_instr;        // instructions per k-step (bn = n_instr * ni_cols)
-    uint32_t total_ksteps;   // ceil(K' / 128)
+    uint32_t total_ksteps;   // ceil(K' / 128): number of 128-byte k-atoms
     uint32_t ksteps_per_chunk;
     uint32_t n_chunks;
+    uint32_t katoms;         // k-atoms per pipeline stage (>= 1): one stage = katoms x (A box + B boxes)
+    uint32_t atom_bytes;     // per CTA: 16 KiB of DB + this CTA's share of the limb tile, for one k-atom
     uint32_t stages;
-    uint32_t stage_bytes;    // per CTA
+    uint32_t stage_bytes;    // per CTA = katoms * atom_bytes
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
     uint32_t n_moduli;
@@ -126,34 +128,49 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         // ===== TMA producer =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            const uint32_t b_rows = p.ni_cols / CG;              // limb-plane rows this CTA stages per instruction
+            const uint32_t b_rows = p.ni_cols / CG;  // limb-plane rows this CTA stages per instruction
             const uint32_t b_bytes = b_rows * GM_BK;
-            // the DB is streamed once (twice when n_tiles == 2: the sibling tile re-reads it from L2)
-            const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
             for (uint32_t u = unit0; u < n_units; u += unit_stride) {
                 const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
+                // the DB streams through L2 once per N tile; only the last N tile of an M tile marks
+                // it evict_first (its siblings, running alongside, re-read it from L2)
+                const uint64_t hintA = (nt + 1 == p.n_tiles) ? ptx::kEvictFirst : ptx::kEvictNormal;
                 const int32_t row0 = (int32_t)((mt * CG + rank) * GM_BM);
-                for (uint32_t ks = 0; ks < p.total_ksteps; ++ks) {
-                    ptx::mbar_wait(&empty[stage], phase ^ 1);
-                    uint8_t* sA = smem + (size_t)stage * p.stage_bytes;
-                    uint8_t* sB = sA + GM_A_BYTES;
-                    const int32_t k0 = (int32_t)(ks * GM_BK);
-                    if constexpr (CG == 1) {
-                        ptx::mbar_arrive_expect_tx(&full[stage], p.stage_bytes);
-                        ptx::tma_load_2d(sA, &tmA, &full[stage], k0, row0, hintA);
-                        for (uint32_t j = 0; j < p.n_instr; ++j)
-                            ptx::tma_load_2d(sB + j * b_bytes, &tmB, &full[stage], k0,
-                                             (int32_t)(nt * p.bn + j * p.ni_cols), ptx::kEvictLast);
-                    } else {
-                        // both CTAs' bytes are counted on the leader's barrier
-                        if (rank == 0) ptx::mbar_arrive_expect_tx(&full[stage], 2 * p.stage_bytes);
-                        const uint32_t bar = ptx::mapa(ptx::smem_u32(&full[stage]), 0);
-                        ptx::tma_load_2d_pair(sA, &tmA, bar, k0, row0, hintA);
-                        for (uint32_t j = 0; j < p.n_instr; ++j)
-                            ptx::tma_load_2d_pair(sB + j * b_bytes, &tmB, bar, k0,
-                                                  (int32_t)(nt * p.bn + j * p.ni_cols + rank * b_rows), ptx::kEvictLast);
+                for (uint32_t c = 0; c < p.n_chunks; ++c) {
+                    const uint32_t ks_begin = c * p.ksteps_per_chunk;
+                    const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
+                    // a stage never straddles a chunk: the last stage of a chunk may hold fewer atoms
+                    for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
+                        const uint32_t na = min(p.katoms, ks_end - ks0);
+                        ptx::mbar_wait(&empty[stage], phase ^ 1);
+                        uint8_t* sbase = smem + (size_t)stage * p.stage_bytes;
+                        uint32_t bar = 0;
+                        if constexpr (CG == 1) {
+                            ptx::mbar_arrive_expect_tx(&full[stage], na * p.atom_bytes);
+                        } else {
+                            // both CTAs' bytes are counted on the leader's barrier
+                            if (rank == 0) ptx::mbar_arrive_expect_tx(&full[stage], 2 * na * p.atom_bytes);
+                            bar = ptx::mapa(ptx::smem_u32(&full[stage]), 0);
+                        }
+                        for (uint32_t a = 0; a < na; ++a) {
+                            uint8_t* sA = sbase + a * p.atom_bytes;
+                            uint8_t* sB = sA + GM_A_BYTES;
+                            const int32_t k0 = (int32_t)((ks0 + a) * GM_BK);
+                            if constexpr (CG == 1) {
+                                ptx::tma_load_2d(sA, &tmA, &full[stage], k0, row0, hintA);
+                                for (uint32_t j = 0; j < p.n_instr; ++j)
+                                    ptx::tma_load_2d(sB + j * b_bytes, &tmB, &full[stage], k0,
+                                                     (int32_t)(nt * p.bn + j * p.ni_cols), ptx::kEvictLast);
+                            } else {
+                                ptx::tma_load_2d_pair(sA, &tmA, bar, k0, row0, hintA);
+                                for (uint32_t j = 0; j < p.n_instr; ++j)
+                                    ptx::tma_load_2d_pair(sB + j * b_bytes, &tmB, bar, k0,
+                                                          (int32_t)(nt * p.bn + j * p.ni_cols + rank * b_rows),
+                                                          ptx::kEvictLast);
+                            }
+                        }
+                        if (++stage == p.stages) { stage = 0; phase ^= 1; }
                     }
-                    if (++stage == p.stages) { stage = 0; phase ^= 1; }
                 }
             }
         }
@@ -172,20 +189,24 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     const uint32_t ks_begin = c * p.ksteps_per_chunk;
                     const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
                     const uint32_t tacc = tmem_base + as * p.bn;
-                    for (uint32_t ks = ks_begin; ks < ks_end; ++ks) {
+                    for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
+                        const uint32_t na = min(p.katoms, ks_end - ks0);
                         ptx::mbar_wait(&full[stage], phase);
                         ptx::tc_fence_after();
-                        const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * p.stage_bytes);
-                        const uint32_t sB = sA + GM_A_BYTES;
-                        const uint64_t dA = make_smem_desc(sA);
-                        for (uint32_t j = 0; j < p.n_instr; ++j) {
-                            const uint64_t dB = make_smem_desc(sB + j * b_bytes);
+                        const uint32_t sbase = ptx::smem_u32(smem + (size_t)stage * p.stage_bytes);
+                        for (uint32_t a = 0; a < na; ++a) {
+                            const uint32_t sA = sbase + a * p.atom_bytes;
+                            const uint32_t sB = sA + GM_A_BYTES;
+                            const uint64_t dA = make_smem_desc(sA);
+                            for (uint32_t j = 0; j < p.n_instr; ++j) {
+                                const uint64_t dB = make_smem_desc(sB + j * b_bytes);
 #pragma unroll
-                            for (uint32_t kk = 0; kk < GM_BK / GM_UMMA_K; ++kk) {
-                                // advancing K inside the swizzle atom = adding the byte offset >> 4
-                                const uint64_t koff = (uint64_t)((kk * GM_UMMA_K) >> 4);
-                                ptx::mma_i8<CG>(tacc + j * p.ni_cols, dA + koff, dB + koff, p.idesc,
-                                                (ks > ks_begin || kk > 0) ? 1u : 0u);
+                                for (uint32_t kk = 0; kk < GM_BK / GM_UMMA_K; ++kk) {
+                                    // advancing K inside the swizzle atom = adding the byte offset >> 4
+                                    const uint64_t koff = (uint64_t)((kk * GM_UMMA_K) >> 4);
+                                    ptx::mma_i8<CG>(tacc + j * p.ni_cols, dA + koff, dB + koff, p.idesc,
+                                                    (ks0 + a > ks_begin || kk > 0) ? 1u : 0u);
+                                }
                             }
                         }
                         // release the smem slot once these MMAs have read it
@@ -213,34 +234,55 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 ptx::mbar_wait(&tmem_full[as], aphase);
                 ptx::tc_fence_after();
                 const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * p.bn;
-                for (uint32_t g = 0; g < p.qt / 4; ++g) {
-                    uint32_t v[4 * LC];
-                    ptx::tmem_ld16(tacc + g * (4 * LC), v);
-                    if constexpr (LC == 5) ptx::tmem_ld4(tacc + g * (4 * LC) + 16, v + 16);
-                    ptx::tmem_ld_wait();
+                // later chunks add to what chunk 0 stored: a fire-and-forget red.add for q = 2^32; for
+                // primes the old words are fetched eight steps (32 query vectors) at a time so that
+                // one global-load latency is paid per batch, not per step
+                constexpr uint32_t kPf = 8;
+                for (uint32_t g0 = 0; g0 < p.qt / 4; g0 += kPf) {
+                    uint32_t old[PRIME ? 4 * kPf : 1];
+                    if constexpr (PRIME) {
+                        if (c > 0) {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const uint32_t q = nt * p.qt + g * 4 + i;
-                        if (q < p.nq && row_ok) {
-                            uint32_t* dst = p.answer + (uint64_t)q * p.rows + row;
-                            uint32_t val;
-                            if constexpr (!PRIME) {
-                                // shifts, wrap mod 2^32 (an s = 4 column would vanish)
-                                val = v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
-                                if (c > 0) val += *dst;
-                            } else {
-                                const uint32_t t = q / p.batch;
-                                const uint32_t pm = p.moduli[t];
-                                uint64_t x = 0;
+                            for (uint32_t i = 0; i < 4 * kPf; ++i) {
+                                const uint32_t q = nt * p.qt + g0 * 4 + i;
+                                old[i] = (q < p.nq && row_ok && g0 * 4 + i < p.qt)
+                                             ? __ldcg(p.answer + (uint64_t)q * p.rows + row) : 0u;
+                            }
+                        }
+                    }
 #pragma unroll
-                                for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
-                                val = barrett_u64(x, pm, p.barrett[t]);
-                                if (c > 0) {
-                                    val += *dst;
-                                    if (val >= pm) val -= pm;
+                    for (uint32_t gg = 0; gg < kPf; ++gg) {
+                        const uint32_t g = g0 + gg;
+                        if (g >= p.qt / 4) break;
+                        uint32_t v[4 * LC];
+                        ptx::tmem_ld16(tacc + g * (4 * LC), v);
+                        if constexpr (LC == 5) ptx::tmem_ld4(tacc + g * (4 * LC) + 16, v + 16);
+                        ptx::tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const uint32_t q = nt * p.qt + g * 4 + i;
+                            if (q < p.nq && row_ok) {
+                                uint32_t* dst = p.answer + (uint64_t)q * p.rows + row;
+                                if constexpr (!PRIME) {
+                                    // shifts, wrap mod 2^32 (an s = 4 column would vanish)
+                                    const uint32_t val =
+                                        v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
+                                    if (c == 0) *dst = val;
+                                    else asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
+                                } else {
+                                    const uint32_t t = q / p.batch;
+                                    const uint32_t pm = p.moduli[t];
+                                    uint64_t x = 0;
+#pragma unroll
+                                    for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
+                                    uint32_t val = barrett_u64(x, pm, p.barrett[t]);
+                                    if (c > 0) {
+                                        val += old[gg * 4 + i];
+                                        if (val >= pm) val -= pm;
+                                    }
+                                    *dst = val;
                                 }
                             }
-                            *dst = val;
                         }
                     }
                 }

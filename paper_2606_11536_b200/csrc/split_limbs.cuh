@@ -18,6 +18,16 @@
 
 namespace vipir {
 
+// 128-bit store that leaves the line in L2 with evict_last priority: the planes are re-read by
+// every M tile of the scan kernel while the DB streams through the same L2.
+__device__ __forceinline__ void st_evict_last(uint8_t* dst, uint4 v) {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(dst), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w), "l"(pol)
+                 : "memory");
+}
+
 // 4x4 byte transpose of four consecutive query words with 8 prmt (2 per element).
 __device__ __forceinline__ void byte_transpose4(uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t L[4]) {
     const uint32_t ab_lo = __byte_perm(a, b, 0x5140);  // a0 b0 a1 b1
@@ -63,7 +73,7 @@ __global__ void __launch_bounds__(256) split_limbs_kernel(const uint32_t* __rest
         for (int s = 0; s < LC; ++s) {
             uint8_t* dst = P + ((uint64_t)q * LC + s) * kp + k0;
             if (k0 + 15 < cols) {
-                *reinterpret_cast<uint4*>(dst) = make_uint4(L[0][s], L[1][s], L[2][s], L[3][s]);
+                st_evict_last(dst, make_uint4(L[0][s], L[1][s], L[2][s], L[3][s]));
             } else {
                 for (int w = 0; w < 4; ++w)
                     for (int e = 0; e < 4; ++e)
@@ -84,8 +94,8 @@ __global__ void __launch_bounds__(256) split_limbs_kernel(const uint32_t* __rest
             }
             uint8_t* dst = P + ((uint64_t)q * LC + s) * kp + 2 * k0;
             if (k0 + 15 < cols) {
-                reinterpret_cast<uint4*>(dst)[0] = make_uint4(o[0], o[1], o[2], o[3]);
-                reinterpret_cast<uint4*>(dst)[1] = make_uint4(o[4], o[5], o[6], o[7]);
+                st_evict_last(dst, make_uint4(o[0], o[1], o[2], o[3]));
+                st_evict_last(dst + 16, make_uint4(o[4], o[5], o[6], o[7]));
             } else {
                 for (int w = 0; w < 8; ++w)
                     for (int e = 0; e < 4; ++e)

@@ -1,6 +1,7 @@
 // vipir_api.cu -- host side of libvipir: plan (step a0), dispatch, C ABI (include/vipir.h).
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -68,6 +69,11 @@ int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint3
     return VIPIR_OK;
 }
 
+// tuning override read at plan time (experiments only; unset = the planner's own choice)
+uint32_t tune_env(const char* name, uint32_t dflt) {
+    const char* v = getenv(name);
+    return (v && *v) ? (uint32_t)strtoul(v, nullptr, 10) : dflt;
+}
 uint32_t round_up(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
 uint32_t ceil_div(uint32_t x, uint32_t m) { return (x + m - 1) / m; }
 
@@ -176,10 +182,23 @@ int plan_gemm(vipir_plan* p, int cg) {
     const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
     g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
-    g.stage_bytes = vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
+    g.atom_bytes = vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
     const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
+    // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes"); VIPIR_TUNE_* override
+    // measured on B200 (profiles/r01_tuning.md): several k-atoms per stage (longer contiguous DB
+    // runs per row, fewer barrier round trips) beat deeper rings of single atoms; keep >= 3 stages
+    uint32_t katoms = (kMaxSmem - overhead) / 3 / g.atom_bytes;
+    if (katoms > 4) katoms = 4;
+    katoms = tune_env("VIPIR_TUNE_KATOMS", katoms);
+    if (katoms < 1) katoms = 1;
+    while (katoms > 1 && 2 * katoms * g.atom_bytes > kMaxSmem - overhead) --katoms;
+    if (katoms > g.ksteps_per_chunk) katoms = g.ksteps_per_chunk;
+    g.katoms = katoms;
+    g.stage_bytes = katoms * g.atom_bytes;
     uint32_t stages = (kMaxSmem - overhead) / g.stage_bytes;
     if (stages > 12) stages = 12;
+    const uint32_t want = tune_env("VIPIR_TUNE_GEMM_STAGES", 0);
+    if (want >= 2 && want < stages) stages = want;
     if (stages < 2) return VIPIR_ERR_UNSUPPORTED;
     g.stages = stages;
     g.acc_stages = (2 * bn <= 512) ? 2u : 1u;
@@ -210,7 +229,9 @@ int plan_gemv(vipir_plan* p) {
     g.kbytes = (uint32_t)p->kbytes;
     g.n_ksteps = (uint32_t)((p->kbytes + vipir::GV_KT - 1) / vipir::GV_KT);
     g.n_blocks = (uint32_t)((p->rows + vipir::GV_R - 1) / vipir::GV_R);
-    g.stages = 6;
+    g.stages = tune_env("VIPIR_TUNE_GEMV_STAGES", 4);  // 4 x 36 KiB in flight per SM measured best
+    if (g.stages < 2) g.stages = 2;
+    if (g.stages > 6) g.stages = 6;
     p->smem_bytes = g.stages * vipir::GV_STAGE_BYTES + 128 + 2 * 8 * g.stages + 2 * vipir::GV_R * 4;
     p->grid = g.n_blocks < (uint32_t)p->num_sms ? g.n_blocks : (uint32_t)p->num_sms;
     // limb planes [4][K'] viewed as u32 elements: box 256 elements (1024 B) x 4 rows
@@ -295,7 +316,9 @@ int vipir_dbmul_plan_ex(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t
 
     if (regime == VIPIR_REGIME_AUTO) {
         if (p->nq == 1 && n_moduli == 0) regime = VIPIR_REGIME_GEMV;
-        else regime = ((uint64_t)p->nq * p->lc > 256 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
+        // measured (profiles/r01_tuning.md): CTA pairs win from 32 query vectors up, where the limb
+        // tile's shared-memory traffic starts to matter; below that one CTA per tile is as fast
+        else regime = ((uint64_t)p->nq * p->lc > 64 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
     }
     p->regime = regime;
 
