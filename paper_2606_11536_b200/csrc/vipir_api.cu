@@ -163,6 +163,8 @@ int plan_gemm(vipir_plan* p, int cg) {
         n_tiles = ceil_div(p->nq, qt_max);
         qt = round_up(ceil_div(p->nq, n_tiles), q_align);
     }
+    const uint32_t qt_force = tune_env("VIPIR_TUNE_QT", 0);
+    if (qt_force >= q_align && qt_force % q_align == 0 && qt_force <= qt_max) qt = qt_force;
     uint32_t bn = qt * lc;
     if (bn > 256) {
         qt = round_up(qt, q_align2);
