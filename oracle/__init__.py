@@ -9,5 +9,6 @@ from .vipir_oracle import (  # noqa: F401
     dbmul,
     dbmul_limbs,
     dbmul_bruteforce,
+    modswitch,
     lib_path,
 )

@@ -81,3 +81,21 @@ def decrypt_answer(A: np.ndarray, s: np.ndarray) -> np.ndarray:
 def worst_case_noise_ok(cols: int) -> bool:
     """|sum_k D[r][k] e_k| <= 255 * 19 * cols must stay below Delta/2 = 2^23."""
     return 255 * 19 * cols < (DELTA >> 1)
+
+
+def decrypt_answer_switched(A_sw: np.ndarray, s: np.ndarray, bits: int = 18) -> np.ndarray:
+    """Decrypt an answer whose words were modulus-switched to 2^bits:
+    same phase computation mod 2^bits with scale Delta' = 2^bits / p."""
+    n = s.size
+    rows = A_sw.shape[1]
+    q2 = 1 << bits
+    delta2 = q2 >> P_BITS
+    out = np.empty(rows, dtype=np.uint8)
+    s_obj = [int(x) for x in s]
+    for r in range(rows):
+        phase = int(A_sw[n, r])
+        for j in range(n):
+            phase += int(A_sw[j, r]) * s_obj[j]
+        phase %= q2
+        out[r] = ((phase + (delta2 >> 1)) // delta2) & 0xFF
+    return out

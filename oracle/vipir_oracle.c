@@ -31,6 +31,9 @@
  *   A  [T][batch][rows] uint32, canonical representative in [0, q_t).
  *   n_moduli == 0 means q = 2^32 (wrapping).
  *
+ *   vipir_oracle_modswitch    NEXT-1 of SURVEY.md section 8(f): the scalar-HE modulus switch
+ *                             2^32 -> 2^bits applied to every answer word.
+ *
  * Parity pins: tests/test_oracle_pins.py (brute force on tiny shapes, closed forms,
  * identity, permutation probe, unit vectors, linearity, toy LWE round trip, CRT).  Nothing
  * in this file is "parity unpinned".
@@ -154,4 +157,25 @@ int vipir_oracle_dbmul_limbs(uint64_t rows, uint64_t cols, uint32_t batch, int d
     }
     for (int j = 0; j < 4; ++j) free(Bj[j]);
     return overflow ? -2 : 0;
+}
+
+/*
+ * Scalar-HE modulus switch (section 5: the ciphertext modulus 2^32 "is reduced to
+ * 2^18 after each scalar-HE folding step"; Appendix D.2: "we reduce the
+ * ciphertext modulus of scalar-HE ciphertexts from 2^32 to p = 2^18 ... equivalent to
+ * introducing an additional rounding error term into each element", |r| < 2^13 in the 2^32
+ * scale, i.e. rounding to nearest).  Plain definition, per word x in [0, 2^32):
+ *     y = round( x * 2^bits / 2^32 )  mod 2^bits,   ties rounded up (reading R19)
+ * written with a multiply and a divide so it can be checked by eye; in place.
+ * 1 <= bits <= 31.  Returns 0, or -1 on a bad argument.
+ */
+int vipir_oracle_modswitch(uint32_t *A, uint64_t n, int bits) {
+    if (!A || bits < 1 || bits > 31) return -1;
+    const uint64_t q_in = 1ull << 32, q_out = 1ull << bits;
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint64_t num = (uint64_t)A[i] * q_out;         /* x * 2^bits < 2^63 */
+        const uint64_t y = (2 * num + q_in) / (2 * q_in);    /* floor(x*2^bits/2^32 + 1/2) */
+        A[i] = (uint32_t)(y % q_out);
+    }
+    return 0;
 }

@@ -49,6 +49,8 @@ def _load():
         lib.vipir_oracle_dbmul.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp, i32]
         lib.vipir_oracle_dbmul_limbs.restype = ctypes.c_int
         lib.vipir_oracle_dbmul_limbs.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp, u64]
+        lib.vipir_oracle_modswitch.restype = ctypes.c_int
+        lib.vipir_oracle_modswitch.argtypes = [vp, u64, i32]
         _lib = lib
     return _lib
 
@@ -103,6 +105,15 @@ def dbmul_limbs(D, Q, moduli=None, k_chunk: int = 32768) -> np.ndarray:
     if rc != 0:
         raise ValueError(f"vipir_oracle_dbmul_limbs failed: {rc}")
     return A
+
+
+def modswitch(A, bits: int = 18) -> np.ndarray:
+    """Scalar-HE modulus switch 2^32 -> 2^bits of every word; returns a copy."""
+    out = np.ascontiguousarray(A, dtype=np.uint32).copy()
+    rc = _load().vipir_oracle_modswitch(_ptr(out), out.size, int(bits))
+    if rc != 0:
+        raise ValueError(f"vipir_oracle_modswitch failed: {rc}")
+    return out
 
 
 def dbmul_bruteforce(D, Q, moduli=None):

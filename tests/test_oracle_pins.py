@@ -267,3 +267,39 @@ def test_rns_primes_are_as_recorded(golden):
     for p in got:
         assert p < (1 << 30) and p % 8192 == 1
         assert all(p % d for d in range(2, 40000))  # trial division: really prime (sqrt(2^30) = 32768)
+
+
+# ---- NEXT-1: scalar-HE modulus switch 2^32 -> 2^18 --------------------
+
+def test_modswitch_is_round_to_nearest_with_bounded_error():
+    from fractions import Fraction
+    xs = np.array([0, 1, 8191, 8192, 8193, 16383, 16384, 16385, 24576, 0x7FFFFFFF, 0x80000000,
+                   0xFFFFDFFF, 0xFFFFE000, 0xFFFFFFFF, 123456789, 4000000000], dtype=np.uint32)
+    ys = oracle.modswitch(xs, 18)
+    for x, y in zip(xs.tolist(), ys.tolist()):
+        exact = Fraction(x * (1 << 18), 1 << 32)
+        want = int(exact + Fraction(1, 2)) % (1 << 18)  # floor(v + 1/2): nearest, ties up (R19)
+        assert y == want, (x, y, want)
+        assert 0 <= y < (1 << 18)
+        err = (x - (y << 14) + (1 << 31)) % (1 << 32) - (1 << 31)  # centred difference mod 2^32
+        assert abs(err) <= 1 << 13  # each rounding error within 2^31/p = 2^13
+    rnd = np.random.default_rng(9).integers(0, 1 << 32, size=5000, dtype=np.uint64).astype(np.uint32)
+    y = oracle.modswitch(rnd, 18).astype(np.int64)
+    err = (rnd.astype(np.int64) - (y << 14) + (1 << 31)) % (1 << 32) - (1 << 31)
+    assert np.abs(err).max() <= 1 << 13
+    assert np.array_equal(oracle.modswitch(np.arange(0, 1 << 20, 1 << 14, dtype=np.uint32), 18),
+                          np.arange(64, dtype=np.uint32))  # exact multiples of 2^14 map exactly
+    assert np.array_equal(oracle.modswitch(rnd, 31), ((rnd.astype(np.uint64) + 1) >> 1).astype(np.uint32) & 0x7FFFFFFF)
+
+
+def test_modswitched_answer_still_decrypts():
+    # |E_round| <= (n+1) * 2^13 must stay below Delta/4 = 2^22: n = 15 is safe
+    cols, rows, n = 512, 40, 15
+    g = rng(77)
+    D = inputs.db_rows(37, rows, cols, 8)
+    s = lwe.keygen(n, g)
+    Q, _ = lwe.simplepir_query(cols, 100, s, g)
+    A = oracle.dbmul(D, Q.reshape(1, n + 1, cols))[0]
+    A18 = oracle.modswitch(A, 18)
+    assert A18.max() < (1 << 18)
+    assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 100])
