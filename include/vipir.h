@@ -92,6 +92,7 @@ typedef struct {
     uint32_t launches;        /* kernels enqueued per vipir_dbmul call */
     uint64_t workspace_bytes; /* limb planes */
     void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
+    uint32_t modswitch_bits;  /* fused output modulus switch in effect (0 = off) */
 } vipir_info;
 
 /*
@@ -140,6 +141,15 @@ int vipir_split_limbs(vipir_plan *plan, const uint32_t *d_query, uint8_t *d_plan
  * workspace (written by the last vipir_dbmul or vipir_split_limbs(plan, q, NULL, ...) call).
  * vipir_dbmul == vipir_split_limbs + vipir_dbmul_scan.  For per-kernel timing and tests. */
 int vipir_dbmul_scan(vipir_plan *plan, const void *d_db, uint32_t *d_answer, void *cuda_stream);
+
+/*
+ * Fuse the scalar-HE modulus switch into the scan kernel's epilogue (section 5: the
+ * ciphertext modulus 2^32 "is reduced to 2^18 after each scalar-HE folding step"
+ * Appendix D.2): every answer word x becomes  round(x * 2^out_bits / 2^32) mod 2^out_bits  (ties
+ * up), saving a pass over the answer.  out_bits in [1, 31]; 0 switches it off (the default).
+ * Only for q = 2^32 plans.  Errors: INVALID_ARG (out_bits > 31), UNSUPPORTED (prime moduli, NAIVE).
+ */
+int vipir_plan_set_modswitch(vipir_plan *plan, uint32_t out_bits);
 
 /* Describe the plan.  Errors: INVALID_ARG. */
 int vipir_plan_info(const vipir_plan *plan, vipir_info *out);

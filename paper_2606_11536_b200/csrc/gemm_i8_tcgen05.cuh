@@ -57,6 +57,7 @@ struct GemmParams {
     uint32_t stage_bytes;    // per CTA = katoms * atom_bytes
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
+    uint32_t ms_bits;        // fused modulus switch 2^32 -> 2^ms_bits of the answer (0 = off; q = 2^32 only)
     uint32_t n_moduli;
     uint32_t moduli[GM_MAX_MODULI];
     uint64_t barrett[GM_MAX_MODULI];  // floor(2^64 / p)
@@ -238,17 +239,19 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 // later chunks add to what chunk 0 stored: a fire-and-forget red.add for q = 2^32; for
                 // primes the old words are fetched eight steps (32 query vectors) at a time so that
                 // one global-load latency is paid per batch, not per step
+                // with the fused modulus switch (q = 2^32 only) the LAST chunk needs the running sum back
+                // to round it: same batched prefetch, once per tile
                 constexpr uint32_t kPf = 8;
+                const bool ms_final = !PRIME && p.ms_bits != 0 && c + 1 == p.n_chunks;
+                const bool need_old = c > 0 && (PRIME || ms_final);
                 for (uint32_t g0 = 0; g0 < p.qt / 4; g0 += kPf) {
-                    uint32_t old[PRIME ? 4 * kPf : 1];
-                    if constexpr (PRIME) {
-                        if (c > 0) {
+                    uint32_t old[4 * kPf];
+                    if (need_old) {
 #pragma unroll
-                            for (uint32_t i = 0; i < 4 * kPf; ++i) {
-                                const uint32_t q = nt * p.qt + g0 * 4 + i;
-                                old[i] = (q < p.nq && row_ok && g0 * 4 + i < p.qt)
-                                             ? __ldcg(p.answer + (uint64_t)q * p.rows + row) : 0u;
-                            }
+                        for (uint32_t i = 0; i < 4 * kPf; ++i) {
+                            const uint32_t q = nt * p.qt + g0 * 4 + i;
+                            old[i] = (q < p.nq && row_ok && g0 * 4 + i < p.qt)
+                                         ? __ldcg(p.answer + (uint64_t)q * p.rows + row) : 0u;
                         }
                     }
 #pragma unroll
@@ -266,10 +269,16 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                 uint32_t* dst = p.answer + (uint64_t)q * p.rows + row;
                                 if constexpr (!PRIME) {
                                     // shifts, wrap mod 2^32 (an s = 4 column would vanish)
-                                    const uint32_t val =
+                                    uint32_t val =
                                         v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
-                                    if (c == 0) *dst = val;
-                                    else asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
+                                    if (ms_final) {
+                                        if (c > 0) val += old[gg * 4 + i];
+                                        *dst = modswitch_word(val, p.ms_bits);
+                                    } else if (c == 0) {
+                                        *dst = val;
+                                    } else {
+                                        asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
+                                    }
                                 } else {
                                     const uint32_t t = q / p.batch;
                                     const uint32_t pm = p.moduli[t];

@@ -36,6 +36,7 @@ struct GemvParams {
     uint32_t n_ksteps;   // ceil(K' / GV_KT)
     uint32_t n_blocks;   // ceil(rows / GV_R)
     uint32_t stages;
+    uint32_t ms_bits;    // fused modulus switch 2^32 -> 2^ms_bits of the answer (0 = off)
     uint32_t* answer;
 };
 
@@ -145,7 +146,10 @@ gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ 
             asm volatile("bar.sync 1, %0;" ::"n"(GV_CWARPS * 32) : "memory");
             if (threadIdx.x < GV_R) {
                 const uint64_t row = (uint64_t)blk * GV_R + threadIdx.x;
-                if (row < p.rows) p.answer[row] = red[threadIdx.x] + red[GV_R + threadIdx.x];
+                if (row < p.rows) {
+                    const uint32_t v = red[threadIdx.x] + red[GV_R + threadIdx.x];
+                    p.answer[row] = p.ms_bits ? modswitch_word(v, p.ms_bits) : v;
+                }
             }
             asm volatile("bar.sync 1, %0;" ::"n"(GV_CWARPS * 32) : "memory");
         }

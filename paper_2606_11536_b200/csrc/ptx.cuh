@@ -233,4 +233,12 @@ __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t* r) {
 }
 
 }  // namespace ptx
+
+// Scalar-HE modulus switch of one answer word, 2^32 -> 2^bits:
+// round(x * 2^bits / 2^32) mod 2^bits, ties up.  bits in [1, 31]; bits == 0 means "off".
+__device__ __forceinline__ uint32_t modswitch_word(uint32_t x, uint32_t bits) {
+    const uint64_t y = ((uint64_t)x + (1ull << (31 - bits))) >> (32 - bits);
+    return (uint32_t)y & ((1u << bits) - 1u);
+}
+
 }  // namespace vipir

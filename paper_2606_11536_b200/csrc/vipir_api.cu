@@ -84,6 +84,7 @@ struct vipir_plan {
     uint32_t batch, db_bits, dl, lc, nq, n_moduli;
     uint32_t moduli[VIPIR_MAX_MODULI];
     uint32_t regime;
+    uint32_t ms_bits;  // fused modulus switch (0 = off)
     int num_sms;
     // workspace
     uint8_t* d_planes;
@@ -368,11 +369,13 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
             attr_set = true;
         }
         p->gv.answer = d_answer;
+        p->gv.ms_bits = p->ms_bits;
         vipir::gemv_b1_kernel<<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
     p->gm.answer = d_answer;
+    p->gm.ms_bits = p->ms_bits;
     return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
 }
 
@@ -426,6 +429,13 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     return VIPIR_OK;
 }
 
+int vipir_plan_set_modswitch(vipir_plan* p, uint32_t out_bits) {
+    if (!p || out_bits > 31) return VIPIR_ERR_INVALID_ARG;
+    if (out_bits != 0 && (p->n_moduli != 0 || p->regime == VIPIR_REGIME_NAIVE)) return VIPIR_ERR_UNSUPPORTED;
+    p->ms_bits = out_bits;
+    return VIPIR_OK;
+}
+
 int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     if (!p || !o) return VIPIR_ERR_INVALID_ARG;
     memset(o, 0, sizeof *o);
@@ -438,6 +448,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     o->grid = p->grid;
     o->workspace_bytes = p->planes_bytes;
     o->d_limb_planes = p->d_planes;
+    o->modswitch_bits = p->ms_bits;
     o->launches = (p->regime == VIPIR_REGIME_NAIVE) ? 1 : 2;
     if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
         o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;

@@ -24,6 +24,7 @@ MAX_MODULI = 4
 # every symbol include/vipir.h declares
 SYMBOLS = (
     "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
+    "vipir_plan_set_modswitch",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
 )
 
@@ -40,6 +41,7 @@ class Info(ctypes.Structure):
         ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32), ("n_tiles", ctypes.c_uint32),
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
         ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
+        ("modswitch_bits", ctypes.c_uint32),
     ]
 
     def as_dict(self):
@@ -84,6 +86,8 @@ def load() -> ctypes.CDLL:
         lib.vipir_split_limbs.argtypes = [vp, vp, vp, vp]
         lib.vipir_dbmul_scan.restype = i
         lib.vipir_dbmul_scan.argtypes = [vp, vp, vp, vp]
+        lib.vipir_plan_set_modswitch.restype = i
+        lib.vipir_plan_set_modswitch.argtypes = [vp, u32]
         lib.vipir_plan_info.restype = i
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
@@ -154,6 +158,11 @@ def dbmul_scan(plan, d_db, d_answer, stream=None):
     _check(load().vipir_dbmul_scan(plan, _ptr(d_db), _ptr(d_answer), _stream_ptr(stream)), "vipir_dbmul_scan")
 
 
+def plan_set_modswitch(plan, out_bits: int):
+    """vipir_plan_set_modswitch: fuse round(x * 2^out_bits / 2^32) into the epilogue (0 = off)."""
+    _check(load().vipir_plan_set_modswitch(plan, out_bits), "vipir_plan_set_modswitch")
+
+
 def plan_info(plan) -> dict:
     info = Info()
     _check(load().vipir_plan_info(plan, ctypes.byref(info)), "vipir_plan_info")
@@ -167,8 +176,10 @@ def destroy(plan):
 class Plan:
     """Context-manager convenience around dbmul_plan / destroy."""
 
-    def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO):
+    def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO, modswitch_bits=0):
         self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime)
+        if modswitch_bits:
+            plan_set_modswitch(self.handle, modswitch_bits)
         self.info = plan_info(self.handle)
 
     def __call__(self, d_db, d_query, d_answer, stream=None):

@@ -261,3 +261,46 @@ def test_toy_lwe_roundtrip_through_the_gpu():
     Q, _ = lwe.simplepir_query(cols, 321, s, g)
     A = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO)[0]
     assert np.array_equal(lwe.decrypt_answer(A, s), D[:, 321])
+
+
+# ---- NEXT-1: fused modulus switch 2^32 -> 2^18 -----------------------
+
+@pytest.mark.parametrize("regime,rows,cols,batch", [
+    (G, 100, 4112, 1), (M1, 300, 1552, 8), (M2, 300, 1552, 40),
+    (M1, 130, 32768 * 2 + 4112, 2), (M2, 260, 32768 + 528, 130),  # several K chunks: the last one rounds
+])
+@pytest.mark.parametrize("bits", [18, 31, 1])
+def test_fused_modswitch(regime, rows, cols, batch, bits):
+    D, Q = make(200 + batch, rows, cols, batch)
+    D[: rows // 2] = 255  # large sums: exercise the wrap before the rounding
+    got, info = run_dbmul(D, Q, None, regime, return_info=True, modswitch_bits=bits)
+    assert info["modswitch_bits"] == bits
+    want = oracle.modswitch(oracle.dbmul(D, Q, None, nthreads=NT), bits)
+    assert_same(got, want)
+    assert got.max() < (1 << bits)
+
+
+def test_modswitch_rejected_for_prime_moduli():
+    ensure_built()
+    with vipir.Plan(256, 256, 2, 8, PRIMES) as plan:
+        with pytest.raises(vipir.VipirError) as e:
+            vipir.plan_set_modswitch(plan.handle, 18)
+        assert e.value.status == vipir.ERR_UNSUPPORTED
+    with vipir.Plan(256, 256, 2) as plan:
+        with pytest.raises(vipir.VipirError) as e:
+            vipir.plan_set_modswitch(plan.handle, 32)
+        assert e.value.status == vipir.ERR_INVALID_ARG
+        vipir.plan_set_modswitch(plan.handle, 18)
+        vipir.plan_set_modswitch(plan.handle, 0)
+        assert vipir.plan_info(plan.handle)["modswitch_bits"] == 0
+
+
+def test_modswitched_gpu_answer_decrypts():
+    from oracle import lwe
+    cols, rows, n = 1024, 200, 15
+    g = np.random.default_rng(6)
+    D = inputs.db_rows(78, rows, cols, 8)
+    s = lwe.keygen(n, g)
+    Q, _ = lwe.simplepir_query(cols, 77, s, g)
+    A18 = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO, modswitch_bits=18)[0]
+    assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 77])
