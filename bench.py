@@ -47,6 +47,18 @@ CONFIGS = {
     "C4_4GiB_B256": (65536, 65536, 256, 8, False),
     "C5_rns_u16_B64x2": (32768, 32768, 64, 16, True),
 }
+# --paper: the paper's own plain-SimplePIR runs (Table 2: B = 32 at 1/4/16/64 GiB,
+# D0 ~ sqrt(D), H100 NVL) and SURVEY.md 8(f) NEXT-2 shapes of the same product; context, not configs
+PAPER_CONFIGS = {
+    "P_1GiB_B32": (32768, 32768, 32, 8, False),
+    "P_4GiB_B32": (65536, 65536, 32, 8, False),
+    "P_16GiB_B32": (131072, 131072, 32, 8, False),
+    "P_64GiB_B32": (262144, 262144, 32, 8, False),
+    "P_64GiB_B1": (262144, 262144, 1, 8, False),
+    "N2_hint_4GiB_B1280": (65536, 65536, 1280, 8, False),
+    "N2_tall_64GiB_B1": (1 << 20, 65536, 1, 8, False),
+}
+PAPER_QPS_H100 = {"P_1GiB_B32": 8244, "P_4GiB_B32": 2201, "P_16GiB_B32": 565, "P_64GiB_B32": 144}
 HEADLINE = "C3_16GiB_B1"
 BATCHED = "C4_4GiB_B256"
 
@@ -160,7 +172,7 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
     import torch
     from paper_2606_11536_b200 import inputs, vipir
     from paper_2606_11536_b200.inputs import device
-    rows, cols, batch, db_bits, prime = CONFIGS[name]
+    rows, cols, batch, db_bits, prime = (CONFIGS.get(name) or PAPER_CONFIGS[name])
     moduli = inputs.rns_primes(SEED) if prime else None
     kb = cols * db_bits // 8
     d_db = device_db[row_offset_bytes: row_offset_bytes + rows * kb].view(rows, kb)
@@ -256,11 +268,12 @@ def run_cuda(args):
     # this rank's row shard of the (world*rows) x cols DB: same stream, offset by the shard's first byte
     r0, _ = shard_rows(rank, world, rows)
     nbytes = rows * cols
-    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    alloc_bytes = max([nbytes] + [r * c * b // 8 for r, c, _, b, _ in PAPER_CONFIGS.values()]) if args.paper else nbytes
+    buf = torch.empty(alloc_bytes, dtype=torch.uint8, device="cuda")
     lib = device._load()
     import ctypes
     key = generator.stream_key(SEED + 1000003 * rank, generator.STREAM_DB) if world > 1 else generator.stream_key(SEED, generator.STREAM_DB)
-    rc = lib.vipir_inputs_fill_bytes(buf.data_ptr(), nbytes, key, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+    rc = lib.vipir_inputs_fill_bytes(buf.data_ptr(), alloc_bytes, key, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
     assert rc == 0
     torch.cuda.synchronize()
 
@@ -292,6 +305,12 @@ def run_cuda(args):
             tensor_bound = name in (BATCHED, "C5_rns_u16_B64x2")
             extra[name] = run_config(name, buf, args.steps, max(3, args.warmup), peaks,
                                      settle_s=1.0 if tensor_bound else 0.0)
+        if args.paper:
+            for name in PAPER_CONFIGS:
+                extra[name] = run_config(name, buf, max(10, args.steps // 5), 3, peaks)
+                if name in PAPER_QPS_H100:
+                    extra[name]["qps_batch32"] = 32.0 / (extra[name]["ms_per_step"] * 1e-3)
+                    extra[name]["paper_qps_h100_nvl"] = PAPER_QPS_H100[name]
         cpu, _ = cpu_baseline(args.cpu_sample_rows, buf, cols)
 
     if rank == 0:
@@ -330,7 +349,7 @@ def run_cuda(args):
                              "ms_per_launch": b["ms_scan_kernel"], "int8_ops_per_launch": b["int8_ops"],
                              "traffic": profiled_traffic("gemm_i8_kernel")},
             }
-        if args.all:
+        if args.all or args.paper:
             line["configs"] = {n: {k: v for k, v in r.items() if k not in ("alg_bytes", "int8_ops")} for n, r in extra.items()}
             line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in ("alg_bytes", "int8_ops")}
         print(json.dumps(line))
@@ -381,6 +400,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--all", action="store_true", help="also time every other BASELINE.json config")
+    ap.add_argument("--paper", action="store_true", help="also time the paper's Table-2 shapes and NEXT-2 shapes (64 GiB DB)")
     ap.add_argument("--cpu-sample-rows", type=int, default=32768)
     ap.add_argument("--ref-sample-rows", type=int, default=4096)
     args = ap.parse_args()

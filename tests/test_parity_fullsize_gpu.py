@@ -124,3 +124,16 @@ def test_fullsize_sampled_rows_and_column_sums(name, device_db):
     d_db, d_q, d_a = run(name, device_db)
     check_sampled_rows(name, d_a)
     check_column_sum_identity(name, d_db, d_a)
+
+
+# ---- NEXT-2 at full size: hint precomputation and a tall 4 GiB layout ---------------------------
+
+CONFIGS["N2_hint_4GiB_B1280"] = (65536, 65536, 1280, 8, None, "mma_2sm")
+CONFIGS["N2_tall_4GiB_B32"] = (1 << 20, 4096, 32, 8, None, "mma_2sm")        # D/D0 = 2^8 tall layout, :331
+
+
+@pytest.mark.parametrize("name", ["N2_hint_4GiB_B1280", "N2_tall_4GiB_B32"])
+def test_next2_fullsize_sampled_rows(name, device_db):
+    d_db, d_q, d_a = run(name, device_db)
+    check_sampled_rows(name, d_a)
+    check_column_sum_identity(name, d_db, d_a)

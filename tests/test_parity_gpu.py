@@ -304,3 +304,53 @@ def test_modswitched_gpu_answer_decrypts():
     Q, _ = lwe.simplepir_query(cols, 77, s, g)
     A18 = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO, modswitch_bits=18)[0]
     assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 77])
+
+
+# ---- NEXT-2: other shapes of the same product ---------------------------------
+
+@pytest.mark.parametrize("rows,cols,batch", [
+    (260, 528, 1281),   # DoublePIR-style B = n+1 = 1281 query vectors: 11 N tiles
+    (4100, 144, 40),    # tall layout, rows >> cols, 17 M-pair tiles, ragged
+    (130, 272, 1280),   # hint precomputation B = n = 1280
+])
+def test_other_shapes_of_the_product(rows, cols, batch):
+    D, Q = make(300 + batch, rows, cols, batch)
+    got, info = run_dbmul(D, Q, None, AUTO, return_info=True)
+    assert info["regime_name"] == "mma_2sm" and info["n_tiles"] == -(-batch // info["tile_queries"])
+    assert_same(got, oracle.dbmul(D, Q, None, nthreads=NT))
+
+
+# ---- seeded random shapes: every regime the planner can pick, ragged everywhere ----------------
+
+def _random_cases(n, seed):
+    g = np.random.default_rng(seed)
+    cases = []
+    for _ in range(n):
+        db_bits = int(g.choice([8, 8, 16]))
+        dl = db_bits // 8
+        rows = int(g.integers(1, 700))
+        cols = int(g.integers(1, 260)) * (16 // dl)          # row bytes a multiple of 16
+        if g.random() < 0.15:
+            cols += (32768 // dl) * int(g.integers(1, 3))      # cross one or two K-chunk seams
+            rows = int(g.integers(1, 200))
+        kind = g.random()
+        if kind < 0.35:
+            moduli = None
+        elif kind < 0.6:
+            moduli = [int(g.integers(2, 1 << 30))]
+        else:
+            moduli = [int(g.integers(2, 1 << 30)) for _ in range(int(g.integers(2, 5)))]
+        batch = int(g.choice([1, 1, 2, 3, 5, 8, 17, 33, 70, 150]))
+        if cols * dl > 40000:
+            batch = min(batch, 8)
+        cases.append((rows, cols, batch, db_bits, moduli))
+    return cases
+
+
+@pytest.mark.parametrize("case", _random_cases(40, 2024), ids=lambda c: f"{c[0]}x{c[1]}xB{c[2]}u{c[3]}m{0 if c[4] is None else len(c[4])}")
+def test_random_shapes_auto(case):
+    rows, cols, batch, db_bits, moduli = case
+    D, Q = make(rows * 31 + cols, rows, cols, batch, db_bits, moduli)
+    if moduli is None:
+        Q[0, 0, : min(cols, 5)] = 0xFFFFFFFF
+    check(D, Q, moduli, AUTO)
