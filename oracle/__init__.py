@@ -8,6 +8,7 @@ from .vipir_oracle import (  # noqa: F401
     build,
     dbmul,
     dbmul_limbs,
+    dbmul_signed,
     dbmul_bruteforce,
     modswitch,
     lib_path,

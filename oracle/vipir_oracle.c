@@ -179,3 +179,36 @@ int vipir_oracle_modswitch(uint32_t *A, uint64_t n, int bits) {
     }
     return 0;
 }
+
+/*
+ * NEXT-3 of SURVEY.md section 8(f): SIGNED database elements (centred plaintexts: the paper's
+ * decryption range is m in [-p/2, p/2)).  Same definition as vipir_oracle_dbmul
+ * with D[r][k] read as a two's-complement int8 (db_bits == 8) or little-endian int16:
+ *   A[t][b][r] = ( sum_k D[r][k] * Q[t][b][k] ) mod q_t,  sum over the (signed) integers,
+ * result canonical in [0, q_t).  Serial; tests only.
+ */
+int vipir_oracle_dbmul_signed(uint64_t rows, uint64_t cols, uint32_t batch, int db_bits,
+                              uint32_t n_moduli, const uint32_t *moduli,
+                              const void *D, const uint32_t *Q, uint32_t *A) {
+    if (!D || !Q || !A || rows == 0 || cols == 0 || batch == 0) return -1;
+    if (db_bits != 8 && db_bits != 16) return -1;
+    if (n_moduli > 0 && !moduli) return -1;
+    const uint32_t T = n_moduli ? n_moduli : 1;
+    for (uint64_t r = 0; r < rows; ++r)
+        for (uint32_t t = 0; t < T; ++t) {
+            const __int128 q = n_moduli ? (__int128)moduli[t] : (((__int128)1) << 32);
+            for (uint32_t b = 0; b < batch; ++b) {
+                const uint32_t *qv = Q + ((uint64_t)t * batch + b) * cols;
+                __int128 acc = 0;
+                for (uint64_t k = 0; k < cols; ++k) {
+                    const uint64_t u = db_at(D, db_bits, r * cols + k);
+                    const int64_t d = (db_bits == 8) ? (int64_t)(int8_t)(uint8_t)u : (int64_t)(int16_t)(uint16_t)u;
+                    acc += (__int128)d * (__int128)qv[k];
+                }
+                __int128 red = acc % q; /* C remainder has the sign of acc */
+                if (red < 0) red += q;
+                A[((uint64_t)t * batch + b) * rows + r] = (uint32_t)(uint64_t)red;
+            }
+        }
+    return 0;
+}

@@ -49,6 +49,8 @@ def _load():
         lib.vipir_oracle_dbmul.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp, i32]
         lib.vipir_oracle_dbmul_limbs.restype = ctypes.c_int
         lib.vipir_oracle_dbmul_limbs.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp, u64]
+        lib.vipir_oracle_dbmul_signed.restype = ctypes.c_int
+        lib.vipir_oracle_dbmul_signed.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp]
         lib.vipir_oracle_modswitch.restype = ctypes.c_int
         lib.vipir_oracle_modswitch.argtypes = [vp, u64, i32]
         _lib = lib
@@ -104,6 +106,20 @@ def dbmul_limbs(D, Q, moduli=None, k_chunk: int = 32768) -> np.ndarray:
         raise OverflowError("an INT32 limb accumulator overflowed; k_chunk too large")
     if rc != 0:
         raise ValueError(f"vipir_oracle_dbmul_limbs failed: {rc}")
+    return A
+
+
+def dbmul_signed(D, Q, moduli=None) -> np.ndarray:
+    """The definition with SIGNED database elements (D given as uint8/uint16 bit patterns or as
+    int8/int16); centred plaintexts."""
+    D = np.ascontiguousarray(D)
+    if D.dtype in (np.int8, np.int16):
+        D = D.view(np.uint8 if D.dtype == np.int8 else np.uint16)
+    D, Q, mods, db_bits, rows, cols, batch, T, A = _prep(D, Q, moduli)
+    rc = _load().vipir_oracle_dbmul_signed(rows, cols, batch, db_bits, 0 if mods is None else T,
+                                           _ptr(mods), _ptr(D), _ptr(Q), _ptr(A))
+    if rc != 0:
+        raise ValueError(f"vipir_oracle_dbmul_signed failed: {rc}")
     return A
 
 

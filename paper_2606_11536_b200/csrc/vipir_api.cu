@@ -28,6 +28,7 @@ int cuda_fail(cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail(e__, #call);      \
     } while (0)
 
+uint32_t tune_env(const char* name, uint32_t dflt);
 constexpr uint32_t kMaxSmem = 232448;  // 227 KiB opt-in dynamic shared memory per CTA
 constexpr uint32_t kChunkBytes = 32768; // 255*255*32768 < 2^31 (R7)
 
@@ -49,7 +50,8 @@ EncodeTiledFn get_encode_fn() {
 
 // 2-D row-major tensor [dim1][dim0] of `esize`-byte elements, row pitch `pitch` bytes.
 int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint32_t esize, uint64_t dim0,
-                 uint64_t dim1, uint64_t pitch, uint32_t box0, uint32_t box1, CUtensorMapSwizzle sw) {
+                 uint64_t dim1, uint64_t pitch, uint32_t box0, uint32_t box1, CUtensorMapSwizzle sw,
+                 CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) {
         snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled entry point not found");
@@ -61,7 +63,7 @@ int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint3
     cuuint32_t estr[2] = {1, 1};
     (void)esize;
     CUresult r = fn(m, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
-                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
         return VIPIR_ERR_CUDA;
@@ -250,7 +252,8 @@ int encode_db_map(vipir_plan* p, const void* d_db) {
                           vipir::GV_KT / 4, vipir::GV_R, CU_TENSOR_MAP_SWIZZLE_NONE);
     else
         rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes, p->rows, p->kbytes,
-                          vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B);
+                          vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B,
+                          (CUtensorMapL2promotion)tune_env("VIPIR_TUNE_L2PROMO", CU_TENSOR_MAP_L2_PROMOTION_L2_256B));
     if (rc == VIPIR_OK) p->tm_db_for = d_db;
     return rc;
 }

@@ -303,3 +303,44 @@ def test_modswitched_answer_still_decrypts():
     A18 = oracle.modswitch(A, 18)
     assert A18.max() < (1 << 18)
     assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 100])
+
+
+# ---- NEXT-3: signed database elements (centred plaintexts) -----------------------
+
+@pytest.mark.parametrize("db_bits", [8, 16])
+@pytest.mark.parametrize("moduli", [None, PRIMES, [97]])
+def test_signed_db_bruteforce_and_relation_to_unsigned(db_bits, moduli):
+    rows, cols, batch = 7, 37, 3
+    Du = inputs.db_rows(91, rows, cols, db_bits)
+    Ds = Du.view(np.int8 if db_bits == 8 else np.int16)
+    Q = inputs.query(91, cols, batch, moduli)
+    Q[0, 0, 0] = 0xFFFFFFFF
+    mods = [Q32] if moduli is None else moduli
+    got = oracle.dbmul_signed(Ds, Q, moduli)
+    for t, q in enumerate(mods):
+        for b in range(batch):
+            for r in range(rows):
+                s = sum(int(Ds[r, k]) * int(Q[t, b, k]) for k in range(cols))  # Python big ints
+                assert int(got[t, b, r]) == s % q
+    # SURVEY.md reading R1: signed and unsigned answers differ by 2^bits * sum of Q over the
+    # elements whose top bit is set
+    unsigned = oracle.dbmul(Du, Q, moduli)
+    top = (Du >> (db_bits - 1)).astype(np.uint8)  # 0/1 mask as a DB of its own
+    corr = oracle.dbmul(top, Q, moduli).astype(object)
+    for t, q in enumerate(mods):
+        assert np.array_equal((unsigned[t].astype(object) - (1 << db_bits) * corr[t]) % q, got[t].astype(object))
+
+
+def test_signed_db_decrypts_to_the_same_bytes():
+    # Delta * 2^8 = 2^32 = 0 mod q: a centred plaintext m and m + 256 decrypt to the same byte,
+    # and the noise term sum_k D[r][k] e_k is about half as large (|D| <= 128 instead of 255)
+    cols, rows, n = 1024, 30, 7
+    g = rng(123)
+    Du = inputs.db_rows(93, rows, cols, 8)
+    s = lwe.keygen(n, g)
+    Q, e = lwe.simplepir_query(cols, 500, s, g)
+    A = oracle.dbmul_signed(Du.view(np.int8), Q.reshape(1, n + 1, cols))[0]
+    assert np.array_equal(lwe.decrypt_answer(A, s), Du[:, 500])
+    noise_signed = np.abs(Du.view(np.int8).astype(np.int64) @ e).max()
+    noise_unsigned = np.abs(Du.astype(np.int64) @ e).max()
+    assert noise_signed < noise_unsigned
