@@ -15,7 +15,7 @@
  * Definition of the result (bit-exact; no tolerance).  For modulus index t < T, query b < batch,
  * row r < rows:
  *     answer[t][b][r] = ( sum_{k < cols} D[r][k] * Q[t][b][k] )  mod q_t
- * D[r][k] the UNSIGNED value of the element, Q the unsigned 32-bit word (any u32 is legal,
+ * D[r][k] the UNSIGNED value of the element (signed int8 after vipir_plan_set_db_signed), Q the unsigned 32-bit word (any u32 is legal,
  * also >= q_t), the sum over the integers, the result canonical in [0, q_t).
  * T = max(mod.count, 1); mod.count == 0 selects q = 2^32.
  *
@@ -93,6 +93,7 @@ typedef struct {
     uint64_t workspace_bytes; /* limb planes */
     void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
     uint32_t modswitch_bits;  /* fused output modulus switch in effect (0 = off) */
+    uint32_t db_signed;       /* 1 if the DB elements are read as two's-complement int8 (vipir_plan_set_db_signed) */
 } vipir_info;
 
 /*
@@ -150,6 +151,18 @@ int vipir_dbmul_scan(vipir_plan *plan, const void *d_db, uint32_t *d_answer, voi
  * Only for q = 2^32 plans.  Errors: INVALID_ARG (out_bits > 31), UNSUPPORTED (prime moduli, NAIVE).
  */
 int vipir_plan_set_modswitch(vipir_plan *plan, uint32_t out_bits);
+
+/*
+ * Read the database elements as SIGNED two's-complement int8 instead of unsigned (centred
+ * plaintexts: the paper's decryption range is m in [-p/2, p/2), Appendix A.1; a
+ * centred DB halves the |m| <= p/2 factor of the LWE noise term sum_k m_k e_k):
+ *     answer[t][b][r] = ( sum_k (int8)D[r][k] * Q[t][b][k] )  mod q_t,  canonical in [0, q_t).
+ * The same bytes in HBM; the tensor-core path switches the A operand format of
+ * tcgen05.mma.kind::i8 to s8, the batch-1 scan uses dp4a.s32.u32.  is_signed: 0 (default) or 1.
+ * Errors: INVALID_ARG (null plan, is_signed > 1), UNSUPPORTED (db_bits == 16: the byte view of a
+ * signed int16 mixes an unsigned low byte with a signed high byte in one operand).
+ */
+int vipir_plan_set_db_signed(vipir_plan *plan, uint32_t is_signed);
 
 /* Describe the plan.  Errors: INVALID_ARG. */
 int vipir_plan_info(const vipir_plan *plan, vipir_info *out);

@@ -58,6 +58,7 @@ struct GemmParams {
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
     uint32_t ms_bits;        // fused modulus switch 2^32 -> 2^ms_bits of the answer (0 = off; q = 2^32 only)
+    uint32_t db_signed;      // DB bytes are s8 (A format s8 in idesc): the s32 accumulators may be negative
     uint32_t n_moduli;
     uint32_t moduli[GM_MAX_MODULI];
     uint64_t barrett[GM_MAX_MODULI];  // floor(2^64 / p)
@@ -282,10 +283,22 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                 } else {
                                     const uint32_t t = q / p.batch;
                                     const uint32_t pm = p.moduli[t];
-                                    uint64_t x = 0;
+                                    uint32_t val;
+                                    if constexpr (LC == 4) {
+                                        // every |P_s| < 2^31 (R7), so the s32 reading is exact for u8 and s8
+                                        // DBs alike and |x| < 2^56; a negative x reduces as p - (|x| mod p)
+                                        int64_t x = 0;
 #pragma unroll
-                                    for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
-                                    uint32_t val = barrett_u64(x, pm, p.barrett[t]);
+                                        for (int s = 0; s < LC; ++s) x += (int64_t)(int32_t)v[i * LC + s] << (8 * s);
+                                        const bool neg = x < 0;
+                                        val = barrett_u64((uint64_t)(neg ? -x : x), pm, p.barrett[t]);
+                                        if (neg && val != 0) val = pm - val;
+                                    } else {
+                                        uint64_t x = 0;  // u16 DB (never signed): up to 2^63 * 1.004
+#pragma unroll
+                                        for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
+                                        val = barrett_u64(x, pm, p.barrett[t]);
+                                    }
                                     if (c > 0) {
                                         val += old[gg * 4 + i];
                                         if (val >= pm) val -= pm;

@@ -48,6 +48,20 @@ __device__ __forceinline__ uint4 lds128(const uint8_t* p) {
     return v;
 }
 
+// one dp4a: four u8 (or, SIGNED, two's-complement s8) DB bytes x four u8 query-limb bytes; the
+// 32-bit accumulator wraps, which is exact mod 2^32 either way
+template <bool SIGNED>
+__device__ __forceinline__ uint32_t dp4a_db(uint32_t d, uint32_t q, uint32_t acc) {
+    if constexpr (SIGNED) {
+        uint32_t r;
+        asm("dp4a.s32.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(d), "r"(q), "r"(acc));
+        return r;
+    } else {
+        return __dp4a(d, q, acc);
+    }
+}
+
+template <bool SIGNED>
 __global__ void __launch_bounds__(GV_THREADS, 1)
 gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ CUtensorMap tmL, GemvParams p) {
     extern __shared__ uint8_t smem_raw[];
@@ -114,10 +128,10 @@ gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ 
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         uint32_t a = acc[rr * 4 + j];
-                        a = __dp4a(d[rr].x, q[j].x, a);
-                        a = __dp4a(d[rr].y, q[j].y, a);
-                        a = __dp4a(d[rr].z, q[j].z, a);
-                        a = __dp4a(d[rr].w, q[j].w, a);
+                        a = dp4a_db<SIGNED>(d[rr].x, q[j].x, a);
+                        a = dp4a_db<SIGNED>(d[rr].y, q[j].y, a);
+                        a = dp4a_db<SIGNED>(d[rr].z, q[j].z, a);
+                        a = dp4a_db<SIGNED>(d[rr].w, q[j].w, a);
                         acc[rr * 4 + j] = a;
                     }
                 }

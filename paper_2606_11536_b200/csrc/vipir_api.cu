@@ -87,6 +87,7 @@ struct vipir_plan {
     uint32_t moduli[VIPIR_MAX_MODULI];
     uint32_t regime;
     uint32_t ms_bits;  // fused modulus switch (0 = off)
+    uint32_t db_signed;  // DB elements are two's-complement int8
     int num_sms;
     // workspace
     uint8_t* d_planes;
@@ -368,17 +369,26 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
     if (p->regime == VIPIR_REGIME_GEMV) {
         static thread_local bool attr_set = false;
         if (!attr_set) {
-            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)kMaxSmem));
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)kMaxSmem));
             attr_set = true;
         }
         p->gv.answer = d_answer;
         p->gv.ms_bits = p->ms_bits;
-        vipir::gemv_b1_kernel<<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        if (p->db_signed)
+            vipir::gemv_b1_kernel<true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        else
+            vipir::gemv_b1_kernel<false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
     p->gm.answer = d_answer;
     p->gm.ms_bits = p->ms_bits;
+    p->gm.db_signed = p->db_signed;
+    // instruction descriptor bits [7,10): A operand format, 0 = u8, 1 = s8 (B stays u8: the limbs)
+    p->gm.idesc = (p->gm.idesc & ~(7u << 7)) | ((p->db_signed ? 1u : 0u) << 7);
     return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
 }
 
@@ -404,6 +414,7 @@ int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32
         np.batch = p->batch;
         np.db_bits = p->db_bits;
         np.n_moduli = p->n_moduli;
+        np.db_signed = p->db_signed;
         for (uint32_t t = 0; t < p->n_moduli; ++t) np.moduli[t] = p->moduli[t];
         vipir::naive_dbmul_kernel<<<dim3(p->grid, p->nq), 128, 0, st>>>(d_db, d_query, d_answer, np);
         CK(cudaGetLastError());
@@ -439,6 +450,13 @@ int vipir_plan_set_modswitch(vipir_plan* p, uint32_t out_bits) {
     return VIPIR_OK;
 }
 
+int vipir_plan_set_db_signed(vipir_plan* p, uint32_t is_signed) {
+    if (!p || is_signed > 1) return VIPIR_ERR_INVALID_ARG;
+    if (is_signed && p->db_bits != 8) return VIPIR_ERR_UNSUPPORTED;
+    p->db_signed = is_signed;
+    return VIPIR_OK;
+}
+
 int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     if (!p || !o) return VIPIR_ERR_INVALID_ARG;
     memset(o, 0, sizeof *o);
@@ -452,6 +470,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     o->workspace_bytes = p->planes_bytes;
     o->d_limb_planes = p->d_planes;
     o->modswitch_bits = p->ms_bits;
+    o->db_signed = p->db_signed;
     o->launches = (p->regime == VIPIR_REGIME_NAIVE) ? 1 : 2;
     if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
         o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;

@@ -24,7 +24,7 @@ MAX_MODULI = 4
 # every symbol include/vipir.h declares
 SYMBOLS = (
     "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
-    "vipir_plan_set_modswitch",
+    "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
 )
 
@@ -41,7 +41,7 @@ class Info(ctypes.Structure):
         ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32), ("n_tiles", ctypes.c_uint32),
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
         ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
-        ("modswitch_bits", ctypes.c_uint32),
+        ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32),
     ]
 
     def as_dict(self):
@@ -88,6 +88,8 @@ def load() -> ctypes.CDLL:
         lib.vipir_dbmul_scan.argtypes = [vp, vp, vp, vp]
         lib.vipir_plan_set_modswitch.restype = i
         lib.vipir_plan_set_modswitch.argtypes = [vp, u32]
+        lib.vipir_plan_set_db_signed.restype = i
+        lib.vipir_plan_set_db_signed.argtypes = [vp, u32]
         lib.vipir_plan_info.restype = i
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
@@ -163,6 +165,11 @@ def plan_set_modswitch(plan, out_bits: int):
     _check(load().vipir_plan_set_modswitch(plan, out_bits), "vipir_plan_set_modswitch")
 
 
+def plan_set_db_signed(plan, is_signed: bool = True):
+    """vipir_plan_set_db_signed: read the u8 DB bytes as two's-complement int8."""
+    _check(load().vipir_plan_set_db_signed(plan, 1 if is_signed else 0), "vipir_plan_set_db_signed")
+
+
 def plan_info(plan) -> dict:
     info = Info()
     _check(load().vipir_plan_info(plan, ctypes.byref(info)), "vipir_plan_info")
@@ -176,10 +183,13 @@ def destroy(plan):
 class Plan:
     """Context-manager convenience around dbmul_plan / destroy."""
 
-    def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO, modswitch_bits=0):
+    def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO, modswitch_bits=0,
+                 db_signed=False):
         self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime)
         if modswitch_bits:
             plan_set_modswitch(self.handle, modswitch_bits)
+        if db_signed:
+            plan_set_db_signed(self.handle, True)
         self.info = plan_info(self.handle)
 
     def __call__(self, d_db, d_query, d_answer, stream=None):

@@ -11,7 +11,7 @@ def ensure_built():
 
 
 def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.REGIME_AUTO, return_info=False,
-              modswitch_bits=0):
+              modswitch_bits=0, db_signed=False):
     """D_host rows x cols (u8/u16), Q_host [T][B][cols] u32 -> answer [T][B][rows] u32 via libvipir."""
     import torch
     ensure_built()
@@ -23,7 +23,7 @@ def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.
     d_db = torch.from_numpy(D_host.view(np.uint8).reshape(rows, -1)).cuda()
     d_q = torch.from_numpy(Q_host.view(np.int32)).cuda()
     d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")  # poison
-    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits) as plan:
+    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits, db_signed) as plan:
         plan(d_db, d_q, d_a)
         torch.cuda.synchronize()
         info = plan.info

@@ -84,6 +84,7 @@ def test_null_out_pointer(lib):
     assert lib.vipir_split_limbs(None, None, None, None) == vipir.ERR_INVALID_ARG
     assert lib.vipir_dbmul_scan(None, None, None, None) == vipir.ERR_INVALID_ARG
     assert lib.vipir_plan_set_modswitch(None, 18) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_plan_set_db_signed(None, 1) == vipir.ERR_INVALID_ARG
 
 
 def test_no_silent_fallback_without_a_gpu(lib):

@@ -306,6 +306,69 @@ def test_modswitched_gpu_answer_decrypts():
     assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 77])
 
 
+# ---- NEXT-3: signed int8 DB (centred plaintexts) ---------------------------------
+
+@pytest.mark.parametrize("regime,rows,cols,batch,moduli", [
+    (G, 100, 4112, 1, None), (NAIVE, 70, 192, 3, None), (NAIVE, 70, 192, 3, PRIMES),
+    (M1, 300, 1552, 8, None), (M2, 300, 1552, 40, None), (M1, 300, 1552, 5, PRIMES), (M2, 300, 1552, 40, PRIMES),
+    (M1, 130, 32768 * 2 + 4112, 2, None), (M2, 260, 32768 + 528, 70, PRIMES),  # K-chunk seams
+    (AUTO, 1024, 1024, 1, None), (AUTO, 260, 1040, 256, None),
+])
+def test_signed_db(regime, rows, cols, batch, moduli):
+    D, Q = make(400 + batch, rows, cols, batch, 8, moduli)
+    D[: rows // 4] = 0x80      # all -128: most negative limb sums, every accumulator at -128*255*K_chunk
+    D[rows // 4: rows // 2] = 0x7F
+    if moduli is None:
+        Q[0, 0, : min(cols, 64)] = 0xFFFFFFFF
+    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, db_signed=True)
+    assert info["db_signed"] == 1
+    assert_same(got, oracle.dbmul_signed(D, Q, moduli))
+    if moduli:
+        for t, pt in enumerate(moduli):
+            assert (got[t] < pt).all()
+
+
+def test_signed_db_all_min_exact_chunk():
+    # every s32 accumulator at its most negative: -128 * 255 * 32768 > -2^31 (R7 holds a fortiori)
+    cols = 32768
+    D = np.full((128, cols), 0x80, dtype=np.uint8)
+    Q = np.full((1, 4, cols), 0xFFFFFFFF, dtype=np.uint32)
+    for regime in (M1, M2):
+        got = run_dbmul(D, Q, None, regime, db_signed=True)
+        assert (got == (-128 * 0xFFFFFFFF * cols) % (1 << 32)).all()
+        p = PRIMES[1]
+        got = run_dbmul(D, Q, [p], regime, db_signed=True)
+        assert (got == (-128 * 0xFFFFFFFF * cols) % p).all()
+
+
+def test_signed_db_with_modswitch_and_lwe():
+    """A centred DB decrypts to the signed byte (m in [-p/2, p/2)); also through the
+    fused modulus switch."""
+    from oracle import lwe
+    cols, rows, n = 1024, 200, 15
+    g = np.random.default_rng(8)
+    D = inputs.db_rows(79, rows, cols, 8)
+    s = lwe.keygen(n, g)
+    Q, _ = lwe.simplepir_query(cols, 500, s, g)
+    A = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO, db_signed=True)[0]
+    assert np.array_equal(lwe.decrypt_answer(A, s), D[:, 500])  # the byte pattern of the signed value mod 2^8
+    A18 = run_dbmul(D, Q.reshape(1, n + 1, cols), None, AUTO, modswitch_bits=18, db_signed=True)[0]
+    assert np.array_equal(lwe.decrypt_answer_switched(A18, s, 18), D[:, 500])
+
+
+def test_signed_db_rejected_for_u16():
+    ensure_built()
+    with vipir.Plan(256, 256, 2, 16) as plan:
+        with pytest.raises(vipir.VipirError) as e:
+            vipir.plan_set_db_signed(plan.handle, True)
+        assert e.value.status == vipir.ERR_UNSUPPORTED
+    with vipir.Plan(256, 256, 2, 8) as plan:
+        vipir.plan_set_db_signed(plan.handle, True)
+        assert vipir.plan_info(plan.handle)["db_signed"] == 1
+        vipir.plan_set_db_signed(plan.handle, False)
+        assert vipir.plan_info(plan.handle)["db_signed"] == 0
+
+
 # ---- NEXT-2: other shapes of the same product (SURVEY.md 8(f)) ---------------------------------
 
 @pytest.mark.parametrize("rows,cols,batch", [
