@@ -13,3 +13,4 @@ from .vipir_oracle import (  # noqa: F401
     modswitch,
     lib_path,
 )
+from .modgemm import modgemm, modgemm_bruteforce, modgemm_lazy  # noqa: F401  (NEXT-4)

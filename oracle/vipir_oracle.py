@@ -18,6 +18,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "vipir_oracle.c"
+_SRCS = [_SRC, _HERE / "vipir_modgemm_oracle.c"]  # NEXT-4: parallel modular GEMMs (own file, same library)
 _LIB = _HERE / "libvipir_oracle.so"
 _lib = None
 
@@ -27,12 +28,12 @@ def lib_path() -> Path:
 
 
 def build(force: bool = False) -> Path:
-    """Compile oracle/vipir_oracle.c with gcc (plain C, -O2, OpenMP for the row loop)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+    """Compile oracle/*.c with gcc (plain C, -O2, OpenMP for the outer loop)."""
+    if force or not _LIB.exists() or any(_LIB.stat().st_mtime < f.stat().st_mtime for f in _SRCS):
         tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
         subprocess.run(
             ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-Wall", "-Wextra",
-             "-o", str(tmp), str(_SRC)],
+             "-o", str(tmp), *map(str, _SRCS)],
             check=True,
         )
         os.replace(tmp, _LIB)
@@ -53,6 +54,10 @@ def _load():
         lib.vipir_oracle_dbmul_signed.argtypes = [u64, u64, u32, i32, u32, vp, vp, vp, vp]
         lib.vipir_oracle_modswitch.restype = ctypes.c_int
         lib.vipir_oracle_modswitch.argtypes = [vp, u64, i32]
+        lib.vipir_oracle_modgemm.restype = ctypes.c_int
+        lib.vipir_oracle_modgemm.argtypes = [u32, u64, u64, u64, u64, u64, vp, vp, vp, vp, vp, i32]
+        lib.vipir_oracle_modgemm_lazy.restype = ctypes.c_int
+        lib.vipir_oracle_modgemm_lazy.argtypes = [u32, u64, u64, u64, u64, u64, vp, vp, vp, vp, vp, u32]
         _lib = lib
     return _lib
 

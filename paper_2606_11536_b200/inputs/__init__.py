@@ -6,6 +6,10 @@ tests / bench alike.  See generator.py for the definition.
 from .generator import (  # noqa: F401
     STREAM_DB,
     STREAM_QUERY,
+    STREAM_MG_H,
+    STREAM_MG_C,
+    STREAM_MG_G,
+    modgemm_operand,
     db_rows,
     query,
     residues,

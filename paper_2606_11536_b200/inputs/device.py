@@ -62,3 +62,18 @@ def query(seed: int, cols: int, batch: int, moduli=None, device="cuda"):
     if rc:
         raise RuntimeError(f"vipir_inputs fill failed: {rc}")
     return t
+
+
+def modgemm_operand(seed: int, stream: int, moduli, n_coeff: int, per_problem: int, device="cuda"):
+    """Device twin of generator.modgemm_operand: [T][n_coeff][per_problem] torch.int32 (u32 bits)."""
+    import torch
+    key = g.stream_key(seed, stream)
+    t = torch.empty((len(moduli), n_coeff, per_problem), dtype=torch.int32, device=device)
+    lib = _load()
+    n = n_coeff * per_problem
+    rc = 0
+    for i, p in enumerate(moduli):
+        rc |= lib.vipir_inputs_fill_mod(t[i].data_ptr(), n, key, i * n, int(p), _stream())
+    if rc:
+        raise RuntimeError(f"vipir_inputs fill failed: {rc}")
+    return t

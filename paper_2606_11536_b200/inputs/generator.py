@@ -29,6 +29,9 @@ _MASK64 = (1 << 64) - 1
 
 STREAM_DB = 1
 STREAM_QUERY = 2
+STREAM_MG_H = 3  # parallel modular GEMMs: H, C, G residues
+STREAM_MG_C = 4
+STREAM_MG_G = 5
 
 
 def _fin(z: np.ndarray) -> np.ndarray:
@@ -96,6 +99,20 @@ def query(seed: int, cols: int, batch: int, moduli=None) -> np.ndarray:
     out = np.empty((len(moduli), batch, cols), dtype=np.uint32)
     for t, p in enumerate(moduli):
         out[t] = residues(key, t * n, n, int(p)).reshape(batch, cols)
+    return out
+
+
+def modgemm_operand(seed: int, stream: int, moduli, n_coeff: int, per_problem: int,
+                    c0: int = 0, nc: int | None = None) -> np.ndarray:
+    """Operand of the parallel modular GEMMs H*C + (0|G): uniform residues mod
+    q_t, flat index ((t*n_coeff + c)*per_problem + i) -> word(key, index) % q_t.  Returns
+    [T][nc][per_problem] uint32 for coefficients [c0, c0+nc) (the caller reshapes the last axis)."""
+    nc = n_coeff - c0 if nc is None else nc
+    key = stream_key(seed, stream)
+    out = np.empty((len(moduli), nc, per_problem), dtype=np.uint32)
+    for t, p in enumerate(moduli):
+        start = (t * n_coeff + c0) * per_problem
+        out[t] = residues(key, start, nc * per_problem, int(p)).reshape(nc, per_problem)
     return out
 
 
