@@ -176,6 +176,84 @@ const char *vipir_status_str(int status);
 /* Last CUDA error string recorded by this library on the calling thread ("" if none). */
 const char *vipir_last_cuda_error(void);
 
+/* ===========================================================================================
+ * Parallel INT32 modular GEMMs of the ring-packing stage
+ *
+ *     Out = H * C + (0 | G)   mod q_t
+ *
+ * PAPER.md:216 (section 3.5.2): after the NTTs, Tiptoe-style packing (eq. (3))
+ * "reduces to (#RNS * N)-parallel ceil(D1/N) x 2B x n INT32 GEMMs with additional modular
+ * reduction computations"; PAPER.md:261-265 (section 4.2) gives the paper's CUDA-core method
+ * (tile-major layout, lazy reduction).  Here the products run on the int8 tensor cores with
+ * both operands split into 8-bit limbs and ONE modular reduction per output word
+ * (csrc/modgemm_i8.cuh).
+ *
+ * One problem per (modulus t < T, NTT coefficient c < NC): an M x ncols x K product of 32-bit
+ * words mod q_t (M = ceil(D1/N), K = n, ncols = 2B), plus G added to the LAST gcols columns.
+ * Definition (bit-exact): for t, c, column j < ncols, row m < M
+ *   Out[t][c][j][m] = ( sum_{k<K} H[t][c][m][k] * C[t][c][j][k]
+ *                       + (j >= ncols-gcols ? G[t][c][j-(ncols-gcols)][m] : 0) )  mod q_t
+ * over the integers, canonical in [0, q_t).  Any u32 input word is legal (also >= q_t).
+ *
+ * Layouts (dense uint32, DEVICE pointers, 16-byte aligned; "tile-major": every problem's
+ * operands contiguous):
+ *   d_H   [T][NC][M][K]       K contiguous      -- the static hint after its NTTs
+ *   d_C   [T][NC][ncols][K]   each column of C contiguous along K
+ *   d_G   [T][NC][gcols][M]   (may be NULL when gcols == 0)
+ *   d_Out [T][NC][ncols][M]
+ * Ownership: the caller owns all four; the plan owns a re-laid-out byte-limb copy of H
+ * (4*T*NC*M*Kp bytes, Kp = K rounded up to 128; written by vipir_modgemm_set_h, after which the
+ * caller may free d_H) and the limb planes of C (4*T*NC*ncols*Kp bytes, rewritten every call).
+ * Execution and errors as for vipir_dbmul: calls only enqueue on `cuda_stream`; one plan must
+ * not be in flight on two streams.
+ * =========================================================================================== */
+typedef struct vipir_modgemm_plan vipir_modgemm_plan;
+
+typedef struct {
+    uint64_t problems;      /* T * NC */
+    uint32_t k_padded;      /* Kp */
+    uint32_t cta_group;     /* 1, or 2 = CTA pairs (tcgen05 cta_group::2, 256-row tiles) */
+    uint32_t tile_cols;     /* ct: columns of C per N tile */
+    uint32_t mma_n;         /* N of one tcgen05.mma = 4 * ct */
+    uint32_t m_tiles, n_tiles; /* per problem */
+    uint32_t n_chunks;      /* K chunks of <= 8192 (int32 accumulation bound 4*255^2*K < 2^31) */
+    uint32_t a_stages, b_stages, acc_stages;
+    uint32_t smem_bytes, grid;
+    uint32_t launches;      /* kernels enqueued per vipir_modgemm call */
+    uint64_t h_limb_bytes, c_limb_bytes;
+    void *d_h_limbs;        /* DEVICE: [T*NC*M][4*Kp] u8, byte (k/128)*512 + i*128 + k%128 of a row = limb i of H[..][k] */
+    void *d_c_limbs;        /* DEVICE: [T*NC][4][ncols][Kp] u8 */
+} vipir_modgemm_info_t;
+
+/*
+ * Build a plan (host; allocates the limb workspaces on the current device).
+ *   moduli  HOST pointer to T values, 2 <= q_t < 2^30 (the paper's RNS primes are < 2^29)
+ * Errors: INVALID_ARG (null, zero size, T > VIPIR_MAX_MODULI, gcols > ncols, modulus out of
+ * range), UNSUPPORTED (M, K or ncols >= 2^24, NC >= 2^28), ARCH, ALLOC, CUDA.
+ */
+int vipir_modgemm_plan_create(vipir_modgemm_plan **out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K,
+                              uint32_t ncols, uint32_t gcols, const uint32_t *moduli);
+
+/* OFFLINE step: split the static hint H into byte limbs in the plan's GEMM-friendly layout (the
+ * paper's "layout transposition before the GEMMs"; H is precomputed offline,
+ * PAPER.md:222).  Must run before the first vipir_modgemm / vipir_modgemm_products. */
+int vipir_modgemm_set_h(vipir_modgemm_plan *plan, const uint32_t *d_H, void *cuda_stream);
+
+/* ONLINE step: enqueue Out = H*C + (0|G) mod q_t: the C limb splitter followed by the tensor-core
+ * kernel.  Errors: INVALID_ARG (null / misaligned pointer, set_h not called), CUDA. */
+int vipir_modgemm(vipir_modgemm_plan *plan, const uint32_t *d_C, const uint32_t *d_G, uint32_t *d_Out,
+                  void *cuda_stream);
+
+/* The two kernels of vipir_modgemm separately (per-kernel timing, tests):
+ * vipir_modgemm == vipir_modgemm_split_c + vipir_modgemm_products. */
+int vipir_modgemm_split_c(vipir_modgemm_plan *plan, const uint32_t *d_C, void *cuda_stream);
+int vipir_modgemm_products(vipir_modgemm_plan *plan, const uint32_t *d_G, uint32_t *d_Out, void *cuda_stream);
+
+int vipir_modgemm_info(const vipir_modgemm_plan *plan, vipir_modgemm_info_t *out);
+
+/* Free the plan and its workspaces.  NULL is a no-op. */
+void vipir_modgemm_destroy(vipir_modgemm_plan *plan);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,277 @@
+// modgemm_host.cuh -- host side (plan, dispatch, C ABI) of the parallel INT32 modular GEMMs
+// Out = H*C + (0|G) mod q_t (include/vipir.h "vipir_modgemm_*"; kernels in modgemm_i8.cuh).
+// Textually included at the end of vipir_api.cu: it uses that file's helpers (CK, tune_env,
+// get_encode_fn, g_cuda_err).
+#pragma once
+#include "modgemm_i8.cuh"
+
+struct vipir_modgemm_plan {
+    uint32_t T, M, K, Kp, ncols, gcols, cg;
+    uint64_t NC, P;
+    uint32_t moduli[VIPIR_MAX_MODULI];
+    int num_sms;
+    uint8_t* d_hp;       // H byte limbs, interleaved per k-atom: [P*M][4*Kp]   (written by vipir_modgemm_set_h)
+    uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
+    uint64_t hp_bytes, cp_bytes;
+    bool h_set;
+    vipir::ModGemmParams mg;
+    uint32_t smem_bytes, grid;
+    CUtensorMap tm_h, tm_c;
+};
+
+namespace {
+
+int make_tmap_nd(CUtensorMap* m, const void* base, uint32_t rank, const uint64_t* dims, const uint64_t* strides_bytes,
+                 const uint32_t* box) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled entry point not found");
+        return VIPIR_ERR_CUDA;
+    }
+    cuuint64_t d[5], s[4];
+    cuuint32_t b[5], e[5];
+    for (uint32_t i = 0; i < rank; ++i) {
+        d[i] = dims[i];
+        b[i] = box[i];
+        e[i] = 1;
+        if (i + 1 < rank) s[i] = strides_bytes[i];
+    }
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, rank, const_cast<void*>(base), d, s, b, e,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled (rank %u) failed: CUresult %d", rank, (int)r);
+        return VIPIR_ERR_CUDA;
+    }
+    return VIPIR_OK;
+}
+
+int plan_modgemm(vipir_modgemm_plan* p) {
+    vipir::ModGemmParams& g = p->mg;
+    memset(&g, 0, sizeof g);
+    const uint32_t cg = p->cg;
+    // N tile: ct C-columns (multiple of 8) -> MMA N = 4*ct <= 256, 7*ct accumulator columns <= 512.
+    // Up to 32 columns a tile keeps two accumulator stages (2*7*32 = 448), so the drain of one
+    // problem overlaps the products of the next.
+    const uint32_t np8 = round_up(p->ncols, 8);
+    uint32_t ct, n_tiles;
+    if (np8 <= 32) {
+        ct = np8;
+        n_tiles = 1;
+    } else {
+        n_tiles = ceil_div(p->ncols, 64);
+        ct = round_up(ceil_div(p->ncols, n_tiles), 8);
+    }
+    const uint32_t ct_force = tune_env("VIPIR_TUNE_MG_CT", 0);
+    if (ct_force >= 8 && ct_force <= 64 && ct_force % 8 == 0) {
+        ct = ct_force;
+        n_tiles = ceil_div(p->ncols, ct);
+    }
+    g.P = (uint32_t)p->P;
+    g.NC = (uint32_t)p->NC;
+    g.M = p->M;
+    g.ncols = p->ncols;
+    g.gcols = p->gcols;
+    g.ct = ct;
+    g.n_tiles = n_tiles;
+    g.m_tiles = ceil_div(p->M, 128u * cg);
+    g.atoms = p->Kp / vipir::MG_BK;
+    g.n_chunks = ceil_div(g.atoms, vipir::MG_MAX_CHUNK_ATOMS);
+    g.atoms_per_chunk = ceil_div(g.atoms, g.n_chunks);
+    g.b_stage_bytes = vipir::MG_BK * ct * (4 / cg);
+    g.b_stages = tune_env("VIPIR_TUNE_MG_BSTAGES", 3);
+    if (g.b_stages < 2) g.b_stages = 2;
+    const uint32_t overhead = 1024 /* alignment */ + vipir::MG_ZERO_BYTES + 512 /* barriers */;
+    const uint32_t left = kMaxSmem - overhead - g.b_stages * g.b_stage_bytes;
+    g.a_stages = left / vipir::MG_A_BYTES;
+    const uint32_t a_force = tune_env("VIPIR_TUNE_MG_ASTAGES", 0);
+    if (a_force >= 2 && a_force < g.a_stages) g.a_stages = a_force;
+    if (g.a_stages < 4) return VIPIR_ERR_UNSUPPORTED;
+    if (g.a_stages > 24) g.a_stages = 24;
+    g.acc_stages = (2 * 7 * ct <= 512) ? 2u : 1u;
+    uint32_t tc = 32;
+    while (tc < g.acc_stages * 7 * ct) tc <<= 1;
+    g.tmem_cols = tc;
+    g.idesc = (2u << 4) /* D = s32 */ | (0u << 7) /* A = u8 */ | (0u << 10) /* B = u8 */ | (((4 * ct) >> 3) << 17) |
+              (((128u * cg) >> 4) << 24);
+    for (uint32_t t = 0; t < p->T; ++t) {
+        const uint32_t q = p->moduli[t];
+        g.moduli[t] = q;
+        g.c32[t] = (uint32_t)((1ull << 32) % q);
+        g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / q);
+    }
+    p->smem_bytes = g.a_stages * vipir::MG_A_BYTES + g.b_stages * g.b_stage_bytes + overhead;
+    const uint64_t units = (uint64_t)p->P * g.m_tiles * g.n_tiles;
+    if (units >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    const uint32_t max_units = (uint32_t)p->num_sms / cg;
+    p->grid = (uint32_t)(units < max_units ? units : max_units) * cg;
+
+    // H limbs: byte matrix [P][M][4*Kp]; box = 128 B x 128 rows of one problem
+    {
+        const uint64_t dims[3] = {4ull * p->Kp, p->M, p->P};
+        const uint64_t str[2] = {4ull * p->Kp, 4ull * p->Kp * p->M};
+        const uint32_t box[3] = {vipir::MG_BK, vipir::MG_BM, 1};
+        int rc = make_tmap_nd(&p->tm_h, p->d_hp, 3, dims, str, box);
+        if (rc != VIPIR_OK) return rc;
+    }
+    // C limb planes [P][4][ncols][Kp]; box = 128 B x ct columns x (4/cg) planes of one problem
+    {
+        const uint64_t dims[4] = {p->Kp, p->ncols, 4, p->P};
+        const uint64_t str[3] = {p->Kp, (uint64_t)p->Kp * p->ncols, 4ull * p->Kp * p->ncols};
+        const uint32_t box[4] = {vipir::MG_BK, ct, 4 / cg, 1};
+        return make_tmap_nd(&p->tm_c, p->d_cp, 4, dims, str, box);
+    }
+}
+
+template <int CG>
+int launch_modgemm(vipir_modgemm_plan* p, cudaStream_t st) {
+    auto kern = vipir::modgemm_i8_kernel<CG>;
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p->grid);
+    cfg.blockDim = dim3(vipir::MG_THREADS);
+    cfg.dynamicSmemBytes = p->smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_h, p->tm_c, p->mg));
+    return VIPIR_OK;
+}
+
+template <bool INTERLEAVED>
+int launch_mg_split(const uint32_t* src, uint8_t* dst, uint64_t n_rows, uint32_t R, uint32_t K, uint32_t Kp,
+                    cudaStream_t st) {
+    const uint64_t threads = n_rows * (Kp / 16);
+    const uint64_t blocks = (threads + 255) / 256;
+    if (blocks >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    vipir::mg_split_kernel<INTERLEAVED><<<(uint32_t)blocks, 256, 0, st>>>(src, dst, n_rows, R, K, Kp);
+    CK(cudaGetLastError());
+    return VIPIR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vipir_modgemm_plan_create(vipir_modgemm_plan** out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K, uint32_t ncols,
+                              uint32_t gcols, const uint32_t* moduli) {
+    if (!out) return VIPIR_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!moduli || T == 0 || T > VIPIR_MAX_MODULI || NC == 0 || M == 0 || K == 0 || ncols == 0 || gcols > ncols)
+        return VIPIR_ERR_INVALID_ARG;
+    for (uint32_t t = 0; t < T; ++t)
+        if (moduli[t] < 2 || moduli[t] >= (1u << 30)) return VIPIR_ERR_INVALID_ARG;
+    if (M >= (1u << 24) || K >= (1u << 24) || ncols >= (1u << 24) || NC >= (1ull << 28)) return VIPIR_ERR_UNSUPPORTED;
+
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    int major = 0, minor = 0, sms = 0;
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CK(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10 || minor != 0) return VIPIR_ERR_ARCH;
+
+    vipir_modgemm_plan* p = new (std::nothrow) vipir_modgemm_plan;
+    if (!p) return VIPIR_ERR_ALLOC;
+    memset(p, 0, sizeof *p);
+    p->T = T;
+    p->NC = NC;
+    p->P = (uint64_t)T * NC;
+    p->M = M;
+    p->K = K;
+    p->Kp = round_up(K, vipir::MG_BK);
+    p->ncols = ncols;
+    p->gcols = gcols;
+    p->num_sms = sms;
+    for (uint32_t t = 0; t < T; ++t) p->moduli[t] = moduli[t];
+    // CTA pairs (one 256-row tile, each CTA staging half of the C limb tile) once the C tile is wide
+    // enough for its shared-memory traffic to matter; VIPIR_TUNE_MG_CG overrides
+    p->cg = (M > 128 && ncols > 16) ? 2u : 1u;
+    const uint32_t cg_force = tune_env("VIPIR_TUNE_MG_CG", 0);
+    if (cg_force == 1 || cg_force == 2) p->cg = cg_force;
+    p->hp_bytes = p->P * M * 4ull * p->Kp;
+    p->cp_bytes = p->P * 4ull * ncols * p->Kp;
+    if (cudaMalloc(&p->d_hp, p->hp_bytes) != cudaSuccess || cudaMalloc(&p->d_cp, p->cp_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        vipir_modgemm_destroy(p);
+        return VIPIR_ERR_ALLOC;
+    }
+    int rc = plan_modgemm(p);
+    if (rc != VIPIR_OK) {
+        vipir_modgemm_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return VIPIR_OK;
+}
+
+int vipir_modgemm_set_h(vipir_modgemm_plan* p, const uint32_t* d_H, void* cuda_stream) {
+    if (!p || !d_H || (reinterpret_cast<uintptr_t>(d_H) & 15)) return VIPIR_ERR_INVALID_ARG;
+    int rc = launch_mg_split<true>(d_H, p->d_hp, p->P * p->M, p->M, p->K, p->Kp, static_cast<cudaStream_t>(cuda_stream));
+    if (rc == VIPIR_OK) p->h_set = true;
+    return rc;
+}
+
+int vipir_modgemm_split_c(vipir_modgemm_plan* p, const uint32_t* d_C, void* cuda_stream) {
+    if (!p || !d_C || (reinterpret_cast<uintptr_t>(d_C) & 15)) return VIPIR_ERR_INVALID_ARG;
+    return launch_mg_split<false>(d_C, p->d_cp, p->P * p->ncols, p->ncols, p->K, p->Kp,
+                                  static_cast<cudaStream_t>(cuda_stream));
+}
+
+int vipir_modgemm_products(vipir_modgemm_plan* p, const uint32_t* d_G, uint32_t* d_Out, void* cuda_stream) {
+    if (!p || !d_Out || (p->gcols > 0 && !d_G)) return VIPIR_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_Out) & 3) || (reinterpret_cast<uintptr_t>(d_G) & 3)) return VIPIR_ERR_INVALID_ARG;
+    if (!p->h_set) return VIPIR_ERR_INVALID_ARG;
+    p->mg.G = d_G;
+    p->mg.out = d_Out;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    return p->cg == 2 ? launch_modgemm<2>(p, st) : launch_modgemm<1>(p, st);
+}
+
+int vipir_modgemm(vipir_modgemm_plan* p, const uint32_t* d_C, const uint32_t* d_G, uint32_t* d_Out, void* cuda_stream) {
+    int rc = vipir_modgemm_split_c(p, d_C, cuda_stream);
+    if (rc != VIPIR_OK) return rc;
+    return vipir_modgemm_products(p, d_G, d_Out, cuda_stream);
+}
+
+int vipir_modgemm_info(const vipir_modgemm_plan* p, vipir_modgemm_info_t* o) {
+    if (!p || !o) return VIPIR_ERR_INVALID_ARG;
+    memset(o, 0, sizeof *o);
+    o->problems = p->P;
+    o->k_padded = p->Kp;
+    o->cta_group = p->cg;
+    o->tile_cols = p->mg.ct;
+    o->mma_n = 4 * p->mg.ct;
+    o->m_tiles = p->mg.m_tiles;
+    o->n_tiles = p->mg.n_tiles;
+    o->n_chunks = p->mg.n_chunks;
+    o->a_stages = p->mg.a_stages;
+    o->b_stages = p->mg.b_stages;
+    o->acc_stages = p->mg.acc_stages;
+    o->smem_bytes = p->smem_bytes;
+    o->grid = p->grid;
+    o->launches = 2;
+    o->h_limb_bytes = p->hp_bytes;
+    o->c_limb_bytes = p->cp_bytes;
+    o->d_h_limbs = p->d_hp;
+    o->d_c_limbs = p->d_cp;
+    return VIPIR_OK;
+}
+
+void vipir_modgemm_destroy(vipir_modgemm_plan* p) {
+    if (!p) return;
+    if (p->d_hp) cudaFree(p->d_hp);
+    if (p->d_cp) cudaFree(p->d_cp);
+    delete p;
+}
+
+}  // extern "C"

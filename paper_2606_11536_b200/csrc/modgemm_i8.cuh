@@ -1,0 +1,337 @@
+// modgemm_i8.cuh -- SURVEY.md 8(f) NEXT-4: VIPIR's parallel INT32 modular GEMMs
+//     Out = H * C + (0 | G)   mod q_t
+// on the int8 tensor cores.
+//
+// PAPER.md:216 (section 3.5.2): "this reduces to (#RNS * N)-parallel ceil(D1/N) x 2B x n INT32
+// GEMMs with additional modular reduction computations"; PAPER.md:261-265 (section 4.2): the
+// paper runs them on CUDA cores in a "tile-major (GEMM-friendly)" layout with lazy reduction
+// (64-bit accumulators, one reduction per 32 multiply-accumulates, primes < 2^29), because on
+// H100 "modulo-q_i arithmetic ... introduces significant overheads ... under tensor-core
+// execution" (:255-257).
+//
+// B200 design.  What is kept from the paper: a GEMM-friendly re-layout
+// of the operands before the GEMMs (:263) and deferred reduction (:265) -- here deferred over
+// the WHOLE K dimension.  What changes: the products run on tcgen05.mma.kind::i8.  Both
+// operands are split into four 8-bit limbs, H = sum_i 2^(8i) H_i, C = sum_j 2^(8j) C_j, so
+//     H*C = sum_{s=0..6} 2^(8s) S_s,     S_s = sum_{i+j=s} H_i * C_j        (over the integers)
+// and every S_s <= 4 * 255^2 * K stays below 2^31 for K <= 8192 per chunk: the int32 TMEM
+// accumulators hold the exact limb sums, one modular reduction per OUTPUT word (the extreme
+// of the paper's lazy reduction).  16 int8 MACs replace one 32x32->64-bit MAC; the B200's int8
+// tensor rate is ~130x its INT32 ALU rate, so the GEMMs become HBM-bound on streaming H.
+//
+// The seven sums are formed without seven separate products: the B operand holds the four
+// limb planes of the C tile stacked along N in the order (j, column), N = 4*ct, and the MMA for
+// H limb i writes its N accumulator columns at TMEM column offset i*ct -- so column block
+// s = i + j of the accumulator receives H_i*C_j, and the four instructions (i = 0..3)
+// overlap-add into 7*ct columns.
+//
+//   warp 0   TMA producer: per k-atom (128 k) one B box (4 limb planes x ct columns x 128 B) and
+//            four A boxes (128 rows x 128 B, one per H limb) into two mbarrier rings;
+//   warp 1   MMA issuer (one thread): per A box four tcgen05.mma (K = 32 each);
+//   warp 2   TMEM allocator;   warps 4-7 epilogue: tcgen05.ld, recombine in u64, two Barrett
+//            reductions, + G, store (coalesced over rows).
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include "gemm_i8_tcgen05.cuh"  // make_smem_desc, barrett_u64
+#include "ptx.cuh"
+#include "split_limbs.cuh"  // byte_transpose4
+
+namespace vipir {
+
+constexpr int MG_BM = 128;      // rows per CTA
+constexpr int MG_BK = 128;      // k per atom = bytes per limb-plane row segment (one 128B swizzle row)
+constexpr int MG_UMMA_K = 32;
+constexpr int MG_THREADS = 256;
+constexpr int MG_A_BYTES = MG_BM * MG_BK;  // 16 KiB: one H limb of one k-atom
+constexpr int MG_ZERO_BYTES = 1024;        // all-zero A operand (one 8-row swizzle atom, aliased by SBO = 0)
+constexpr int MG_MAX_MODULI = 4;
+constexpr uint32_t MG_MAX_CHUNK_ATOMS = 64;  // 4 * 255^2 * 8192 < 2^31
+
+struct ModGemmParams {
+    uint32_t P;        // problems = T * NC
+    uint32_t NC;       // problems per modulus (modulus index = problem / NC)
+    uint32_t M, ncols, gcols;
+    uint32_t ct;       // C columns per N tile (multiple of 8); MMA N = 4*ct; accumulator columns = 7*ct
+    uint32_t m_tiles, n_tiles;  // per problem
+    uint32_t atoms;    // k-atoms = Kp / 128
+    uint32_t atoms_per_chunk, n_chunks;
+    uint32_t a_stages, b_stages, b_stage_bytes;  // per CTA
+    uint32_t tmem_cols, acc_stages;
+    uint32_t idesc;
+    uint32_t moduli[MG_MAX_MODULI];
+    uint32_t c32[MG_MAX_MODULI];      // 2^32 mod q_t
+    uint64_t barrett[MG_MAX_MODULI];  // floor(2^64 / q_t)
+    const uint32_t* G;                // [P][gcols][M] or nullptr
+    uint32_t* out;                    // [P][ncols][M]
+};
+
+// ---- operand re-layout (the paper's "layout transposition before the GEMMs", :263) -------------
+// X [P][R][K] u32  ->  byte limbs.  One thread = 16 consecutive k of one row.
+//   INTERLEAVED (H, the static hint; written once, offline):
+//       Hp[(p*R + r)][ (k/128)*512 + i*128 + k%128 ] = byte i of X[p][r][k]      row pitch 4*Kp
+//     i.e. per row the four limb segments of one k-atom are adjacent: the (atom, limb) boxes the
+//     kernel loads in sequence are consecutive 128-byte column blocks of one byte matrix.
+//   planes (C, every call):
+//       Cp[((p*4 + i)*R + r)][k] = byte i of X[p][r][k]                           row pitch Kp
+// Kp = K rounded up to 128; the padding is written as zeros.
+template <bool INTERLEAVED>
+__global__ void __launch_bounds__(256) mg_split_kernel(const uint32_t* __restrict__ X, uint8_t* __restrict__ out,
+                                                       uint64_t n_rows /* P*R */, uint32_t R, uint32_t K,
+                                                       uint32_t Kp) {
+    const uint32_t groups = Kp / 16;
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= n_rows * groups) return;
+    const uint64_t row = gid / groups;
+    const uint32_t k0 = (uint32_t)(gid % groups) * 16;
+    const uint32_t* src = X + row * K + k0;
+    uint32_t L[4][4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        uint32_t t[4] = {0, 0, 0, 0};
+        if (k0 + 4 * w + 3 < K && (K & 3) == 0) {
+            const uint4 v = *reinterpret_cast<const uint4*>(src + 4 * w);
+            t[0] = v.x; t[1] = v.y; t[2] = v.z; t[3] = v.w;
+        } else {
+            for (int e = 0; e < 4; ++e)
+                if (k0 + 4 * w + e < K) t[e] = src[4 * w + e];
+        }
+        byte_transpose4(t[0], t[1], t[2], t[3], L[w]);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        uint8_t* dst;
+        if constexpr (INTERLEAVED) {
+            dst = out + row * (4ull * Kp) + (k0 / MG_BK) * (4 * MG_BK) + i * MG_BK + (k0 % MG_BK);
+        } else {
+            const uint64_t p = row / R, r = row % R;
+            dst = out + ((p * 4 + i) * R + r) * (uint64_t)Kp + k0;
+        }
+        *reinterpret_cast<uint4*>(dst) = make_uint4(L[0][i], L[1][i], L[2][i], L[3][i]);
+    }
+}
+
+// zero operand: every 8-row group aliases the same 1 KiB of zeros (stride byte offset 0)
+__device__ __forceinline__ uint64_t make_smem_desc_zero(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+
+// (lo + 2^32 * hi) mod q for lo < 2^57, hi < 2^49, q < 2^30: reduce hi, fold with 2^32 mod q
+__device__ __forceinline__ uint64_t mg_fold(uint64_t lo, uint64_t hi, uint32_t q, uint64_t bm, uint32_t c32) {
+    const uint32_t hr = barrett_u64(hi, q, bm);
+    return lo + (uint64_t)hr * c32;  // < 2^57 + 2^60
+}
+
+template <int CG>
+__global__ void __launch_bounds__(MG_THREADS, 1)
+modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, ModGemmParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* sA_ring = smem;
+    uint8_t* sB_ring = sA_ring + (size_t)p.a_stages * MG_A_BYTES;
+    uint8_t* sZero = sB_ring + (size_t)p.b_stages * p.b_stage_bytes;
+    uint64_t* fullA = reinterpret_cast<uint64_t*>(sZero + MG_ZERO_BYTES);
+    uint64_t* emptyA = fullA + p.a_stages;
+    uint64_t* fullB = emptyA + p.a_stages;
+    uint64_t* emptyB = fullB + p.b_stages;
+    uint64_t* tmem_full = emptyB + p.b_stages;  // [2]
+    uint64_t* tmem_empty = tmem_full + 2;       // [2]
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
+    const uint32_t unit0 = (CG == 2) ? ptx::cluster_id_x() : blockIdx.x;
+    const uint32_t unit_stride = (CG == 2) ? ptx::num_clusters_x() : gridDim.x;
+    const uint32_t tiles_per_problem = p.m_tiles * p.n_tiles;
+    const uint32_t n_units = p.P * tiles_per_problem;
+    const uint32_t acc_cols = 7 * p.ct;
+
+    // the zero operand (generic-proxy writes, made visible to the tensor core's async proxy)
+    for (uint32_t i = threadIdx.x; i < MG_ZERO_BYTES / 4; i += MG_THREADS) reinterpret_cast<uint32_t*>(sZero)[i] = 0u;
+    ptx::fence_proxy_async();
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmA);
+        ptx::prefetch_tmap(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        for (uint32_t s = 0; s < p.a_stages; ++s) {
+            ptx::mbar_init(&fullA[s], 1);
+            ptx::mbar_init(&emptyA[s], 1);
+        }
+        for (uint32_t s = 0; s < p.b_stages; ++s) {
+            ptx::mbar_init(&fullB[s], 1);
+            ptx::mbar_init(&emptyB[s], 1);
+        }
+        for (uint32_t a = 0; a < 2; ++a) {
+            ptx::mbar_init(&tmem_full[a], 1);
+            ptx::mbar_init(&tmem_empty[a], 4 * CG);
+        }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc<CG>(tmem_ptr, p.tmem_cols);
+        ptx::tmem_relinquish<CG>();
+    }
+    ptx::tc_fence_before();
+    if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            uint32_t sa = 0, pa = 0, sb = 0, pb = 0;
+            // H is streamed once when there is a single N tile; sibling N tiles re-read it from L2
+            const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+            for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+                const uint32_t prob = u / tiles_per_problem, rem = u % tiles_per_problem;
+                const uint32_t mt = rem / p.n_tiles, nt = rem % p.n_tiles;
+                const int32_t row0 = (int32_t)((mt * CG + rank) * MG_BM);
+                for (uint32_t a = 0; a < p.atoms; ++a) {
+                    ptx::mbar_wait(&emptyB[sb], pb ^ 1);
+                    uint8_t* dB = sB_ring + (size_t)sb * p.b_stage_bytes;
+                    if constexpr (CG == 1) {
+                        ptx::mbar_arrive_expect_tx(&fullB[sb], p.b_stage_bytes);
+                        ptx::tma_load_4d(dB, &tmB, &fullB[sb], (int32_t)(a * MG_BK), (int32_t)(nt * p.ct), 0,
+                                         (int32_t)prob, ptx::kEvictNormal);
+                    } else {
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(&fullB[sb], 2 * p.b_stage_bytes);
+                        // this CTA stages limb planes j = 2*rank, 2*rank+1: its half of the N = 4*ct rows
+                        ptx::tma_load_4d_pair(dB, &tmB, ptx::mapa(ptx::smem_u32(&fullB[sb]), 0), (int32_t)(a * MG_BK),
+                                              (int32_t)(nt * p.ct), (int32_t)(2 * rank), (int32_t)prob,
+                                              ptx::kEvictNormal);
+                    }
+                    if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
+#pragma unroll 1
+                    for (uint32_t i = 0; i < 4; ++i) {
+                        ptx::mbar_wait(&emptyA[sa], pa ^ 1);
+                        uint8_t* dA = sA_ring + (size_t)sa * MG_A_BYTES;
+                        const int32_t kb = (int32_t)((a * 4 + i) * MG_BK);
+                        if constexpr (CG == 1) {
+                            ptx::mbar_arrive_expect_tx(&fullA[sa], MG_A_BYTES);
+                            ptx::tma_load_3d(dA, &tmA, &fullA[sa], kb, row0, (int32_t)prob, hintA);
+                        } else {
+                            if (rank == 0) ptx::mbar_arrive_expect_tx(&fullA[sa], 2 * MG_A_BYTES);
+                            ptx::tma_load_3d_pair(dA, &tmA, ptx::mapa(ptx::smem_u32(&fullA[sa]), 0), kb, row0,
+                                                  (int32_t)prob, hintA);
+                        }
+                        if (++sa == p.a_stages) { sa = 0; pa ^= 1; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (leader CTA of the pair only) =====
+        if (rank == 0 && lane == 0) {
+            uint32_t sa = 0, pa = 0, sb = 0, pb = 0, acc_it = 0;
+            const uint64_t dZ = make_smem_desc_zero(ptx::smem_u32(sZero));
+            for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+                for (uint32_t c = 0; c < p.n_chunks; ++c, ++acc_it) {
+                    const uint32_t as = acc_it % p.acc_stages;
+                    const uint32_t aphase = (acc_it / p.acc_stages) & 1;
+                    if constexpr (CG == 2) ptx::mbar_wait_cluster(&tmem_empty[as], aphase ^ 1);
+                    else ptx::mbar_wait(&tmem_empty[as], aphase ^ 1);
+                    ptx::tc_fence_after();
+                    const uint32_t a_begin = c * p.atoms_per_chunk;
+                    const uint32_t a_end = min(p.atoms, a_begin + p.atoms_per_chunk);
+                    const uint32_t tacc = tmem_base + as * acc_cols;
+                    for (uint32_t a = a_begin; a < a_end; ++a) {
+                        ptx::mbar_wait(&fullB[sb], pb);
+                        ptx::tc_fence_after();
+                        const uint64_t dB = make_smem_desc(ptx::smem_u32(sB_ring + (size_t)sb * p.b_stage_bytes));
+#pragma unroll 1
+                        for (uint32_t i = 0; i < 4; ++i) {
+                            ptx::mbar_wait(&fullA[sa], pa);
+                            ptx::tc_fence_after();
+                            const uint64_t dA = make_smem_desc(ptx::smem_u32(sA_ring + (size_t)sa * MG_A_BYTES));
+                            const bool first = (a == a_begin && i == 0);
+                            // blocks 3..6 start at zero (0 * anything), then H_0*C overwrites blocks 0..3
+                            if (first) ptx::mma_i8<CG>(tacc + 3 * p.ct, dZ, dB, p.idesc, 0u);
+#pragma unroll
+                            for (uint32_t kk = 0; kk < MG_BK / MG_UMMA_K; ++kk) {
+                                const uint64_t koff = (uint64_t)((kk * MG_UMMA_K) >> 4);
+                                ptx::mma_i8<CG>(tacc + i * p.ct, dA + koff, dB + koff, p.idesc,
+                                                (first && kk == 0) ? 0u : 1u);
+                            }
+                            if constexpr (CG == 2) ptx::tc_commit_pair(&emptyA[sa], 3);
+                            else ptx::tc_commit(&emptyA[sa]);
+                            if (++sa == p.a_stages) { sa = 0; pa ^= 1; }
+                        }
+                        if constexpr (CG == 2) ptx::tc_commit_pair(&emptyB[sb], 3);
+                        else ptx::tc_commit(&emptyB[sb]);
+                        if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
+                    }
+                    if constexpr (CG == 2) ptx::tc_commit_pair(&tmem_full[as], 3);
+                    else ptx::tc_commit(&tmem_full[as]);
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue warps: lane quarter = warp % 4 =====
+        const uint32_t quarter = warp & 3;
+        const uint32_t g0 = p.ncols - p.gcols;
+        uint32_t acc_it = 0;
+        for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+            const uint32_t prob = u / tiles_per_problem, rem = u % tiles_per_problem;
+            const uint32_t mt = rem / p.n_tiles, nt = rem % p.n_tiles;
+            const uint32_t row = (mt * CG + rank) * MG_BM + quarter * 32 + lane;
+            const bool row_ok = row < p.M;
+            const uint32_t t = prob / p.NC;
+            const uint32_t q = p.moduli[t], c32 = p.c32[t];
+            const uint64_t bm = p.barrett[t];
+            for (uint32_t c = 0; c < p.n_chunks; ++c, ++acc_it) {
+                const uint32_t as = acc_it % p.acc_stages;
+                const uint32_t aphase = (acc_it / p.acc_stages) & 1;
+                ptx::mbar_wait(&tmem_full[as], aphase);
+                ptx::tc_fence_after();
+                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols;
+                for (uint32_t g = 0; g < p.ct / 8; ++g) {
+                    uint32_t v[7][8];
+#pragma unroll
+                    for (int s = 0; s < 7; ++s) ptx::tmem_ld8(tacc + s * p.ct + g * 8, v[s]);
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const uint32_t col = nt * p.ct + g * 8 + e;
+                        if (col < p.ncols && row_ok) {
+                            // sum_s 2^(8s) S_s, S_s < 2^31 (one K chunk): low four limbs < 2^57, high three < 2^49
+                            const uint64_t lo = (uint64_t)v[0][e] + ((uint64_t)v[1][e] << 8) + ((uint64_t)v[2][e] << 16) +
+                                                ((uint64_t)v[3][e] << 24);
+                            const uint64_t hi = (uint64_t)v[4][e] + ((uint64_t)v[5][e] << 8) + ((uint64_t)v[6][e] << 16);
+                            uint64_t x = mg_fold(lo, hi, q, bm, c32);
+                            uint32_t* dst = p.out + ((uint64_t)prob * p.ncols + col) * p.M + row;
+                            if (c == 0) {
+                                if (col >= g0) x += p.G[((uint64_t)prob * p.gcols + (col - g0)) * p.M + row];  // (0 | G)
+                            } else {
+                                x += *dst;  // earlier K chunks, already reduced
+                            }
+                            *dst = barrett_u64(x, q, bm);
+                        }
+                    }
+                }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if constexpr (CG == 2) ptx::mbar_arrive_cluster(&tmem_empty[as], 0);
+                    else ptx::mbar_arrive(&tmem_empty[as]);
+                }
+            }
+        }
+    }
+
+    // ===== teardown =====
+    ptx::tc_fence_before();
+    if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc<CG>(tmem_base, p.tmem_cols);
+    }
+}
+
+}  // namespace vipir

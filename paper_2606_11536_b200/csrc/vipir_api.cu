@@ -499,3 +499,5 @@ void vipir_destroy(vipir_plan* p) {
 }
 
 }  // extern "C"
+
+#include "modgemm_host.cuh"  // vipir_modgemm_* (parallel INT32 modular GEMMs, NEXT-4)

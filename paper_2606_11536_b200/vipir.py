@@ -26,6 +26,8 @@ SYMBOLS = (
     "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
     "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
+    "vipir_modgemm_plan_create", "vipir_modgemm_set_h", "vipir_modgemm", "vipir_modgemm_split_c",
+    "vipir_modgemm_products", "vipir_modgemm_info", "vipir_modgemm_destroy",
 )
 
 
@@ -48,6 +50,20 @@ class Info(ctypes.Structure):
         d = {k: getattr(self, k) for k, _ in self._fields_}
         d["regime_name"] = REGIME_NAMES.get(d["regime"], "?")
         return d
+
+
+class ModGemmInfo(ctypes.Structure):
+    _fields_ = [
+        ("problems", ctypes.c_uint64), ("k_padded", ctypes.c_uint32), ("cta_group", ctypes.c_uint32),
+        ("tile_cols", ctypes.c_uint32), ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32),
+        ("n_tiles", ctypes.c_uint32), ("n_chunks", ctypes.c_uint32), ("a_stages", ctypes.c_uint32),
+        ("b_stages", ctypes.c_uint32), ("acc_stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
+        ("grid", ctypes.c_uint32), ("launches", ctypes.c_uint32), ("h_limb_bytes", ctypes.c_uint64),
+        ("c_limb_bytes", ctypes.c_uint64), ("d_h_limbs", ctypes.c_void_p), ("d_c_limbs", ctypes.c_void_p),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 class VipirError(RuntimeError):
@@ -94,6 +110,20 @@ def load() -> ctypes.CDLL:
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
         lib.vipir_destroy.argtypes = [vp]
+        lib.vipir_modgemm_plan_create.restype = i
+        lib.vipir_modgemm_plan_create.argtypes = [pp, u32, u64, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32)]
+        lib.vipir_modgemm_set_h.restype = i
+        lib.vipir_modgemm_set_h.argtypes = [vp, vp, vp]
+        lib.vipir_modgemm.restype = i
+        lib.vipir_modgemm.argtypes = [vp, vp, vp, vp, vp]
+        lib.vipir_modgemm_split_c.restype = i
+        lib.vipir_modgemm_split_c.argtypes = [vp, vp, vp]
+        lib.vipir_modgemm_products.restype = i
+        lib.vipir_modgemm_products.argtypes = [vp, vp, vp, vp]
+        lib.vipir_modgemm_info.restype = i
+        lib.vipir_modgemm_info.argtypes = [vp, ctypes.POINTER(ModGemmInfo)]
+        lib.vipir_modgemm_destroy.restype = None
+        lib.vipir_modgemm_destroy.argtypes = [vp]
         lib.vipir_status_str.restype = ctypes.c_char_p
         lib.vipir_status_str.argtypes = [i]
         lib.vipir_last_cuda_error.restype = ctypes.c_char_p
@@ -201,6 +231,80 @@ class Plan:
     def close(self):
         if self.handle is not None:
             destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ---- parallel INT32 modular GEMMs  Out = H*C + (0|G) mod q_t  (include/vipir.h, NEXT-4) ----------
+
+def modgemm_plan_create(T: int, NC: int, M: int, K: int, ncols: int, gcols: int, moduli):
+    """vipir_modgemm_plan_create; returns the opaque plan handle."""
+    handle = ctypes.c_void_p()
+    arr = (ctypes.c_uint32 * max(len(moduli), 1))(*[int(m) for m in moduli])
+    if len(moduli) != T:
+        raise ValueError(f"{len(moduli)} moduli for T = {T}")
+    _check(load().vipir_modgemm_plan_create(ctypes.byref(handle), T, NC, M, K, ncols, gcols, arr),
+           "vipir_modgemm_plan_create")
+    return handle
+
+
+def modgemm_set_h(plan, d_H, stream=None):
+    """vipir_modgemm_set_h: the offline re-layout of the static hint H [T][NC][M][K] u32."""
+    _check(load().vipir_modgemm_set_h(plan, _ptr(d_H), _stream_ptr(stream)), "vipir_modgemm_set_h")
+
+
+def modgemm(plan, d_C, d_G, d_Out, stream=None):
+    """vipir_modgemm: enqueue Out = H*C + (0|G) mod q_t (C splitter + tensor-core kernel)."""
+    g = ctypes.c_void_p(None) if d_G is None else _ptr(d_G)
+    _check(load().vipir_modgemm(plan, _ptr(d_C), g, _ptr(d_Out), _stream_ptr(stream)), "vipir_modgemm")
+
+
+def modgemm_split_c(plan, d_C, stream=None):
+    _check(load().vipir_modgemm_split_c(plan, _ptr(d_C), _stream_ptr(stream)), "vipir_modgemm_split_c")
+
+
+def modgemm_products(plan, d_G, d_Out, stream=None):
+    g = ctypes.c_void_p(None) if d_G is None else _ptr(d_G)
+    _check(load().vipir_modgemm_products(plan, g, _ptr(d_Out), _stream_ptr(stream)), "vipir_modgemm_products")
+
+
+def modgemm_info(plan) -> dict:
+    info = ModGemmInfo()
+    _check(load().vipir_modgemm_info(plan, ctypes.byref(info)), "vipir_modgemm_info")
+    return info.as_dict()
+
+
+def modgemm_destroy(plan):
+    load().vipir_modgemm_destroy(plan)
+
+
+class ModGemmPlan:
+    """Context-manager convenience around modgemm_plan_create / modgemm_destroy."""
+
+    def __init__(self, T, NC, M, K, ncols, gcols, moduli):
+        self.handle = modgemm_plan_create(T, NC, M, K, ncols, gcols, moduli)
+        self.info = modgemm_info(self.handle)
+
+    def set_h(self, d_H, stream=None):
+        modgemm_set_h(self.handle, d_H, stream)
+
+    def __call__(self, d_C, d_G, d_Out, stream=None):
+        modgemm(self.handle, d_C, d_G, d_Out, stream)
+
+    def close(self):
+        if self.handle is not None:
+            modgemm_destroy(self.handle)
             self.handle = None
 
     def __enter__(self):
