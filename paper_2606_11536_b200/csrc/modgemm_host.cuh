@@ -94,10 +94,11 @@ int plan_modgemm(vipir_modgemm_plan* p) {
     g.tmem_cols = tc;
     g.idesc = (2u << 4) /* D = s32 */ | (0u << 7) /* A = u8 */ | (0u << 10) /* B = u8 */ | (((4 * ct) >> 3) << 17) |
               (((128u * cg) >> 4) << 24);
+    g.dbg = tune_env("VIPIR_TUNE_MG_DBG", 0);
     for (uint32_t t = 0; t < p->T; ++t) {
         const uint32_t q = p->moduli[t];
         g.moduli[t] = q;
-        g.c32[t] = (uint32_t)((1ull << 32) % q);
+        for (int s = 0; s < 3; ++s) g.w[t][s] = (uint32_t)((1ull << (32 + 8 * s)) % q);
         g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / q);
     }
     p->smem_bytes = g.a_stages * vipir::MG_A_BYTES + g.b_stages * g.b_stage_bytes + overhead;

@@ -28,8 +28,9 @@
 //   warp 0   TMA producer: per k-atom (128 k) one B box (4 limb planes x ct columns x 128 B) and
 //            four A boxes (128 rows x 128 B, one per H limb) into two mbarrier rings;
 //   warp 1   MMA issuer (one thread): per A box four tcgen05.mma (K = 32 each);
-//   warp 2   TMEM allocator;   warps 4-7 epilogue: tcgen05.ld, recombine in u64, two Barrett
-//            reductions, + G, store (coalesced over rows).
+//   warp 2   TMEM allocator;   warps 4-11 epilogue: tcgen05.ld, recombine in u64 (shifts for the
+//            low four sums, 2^(8s) mod q weights for the high three), + G, one Barrett reduction,
+//            store (coalesced over rows).
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -42,7 +43,8 @@ namespace vipir {
 constexpr int MG_BM = 128;      // rows per CTA
 constexpr int MG_BK = 128;      // k per atom = bytes per limb-plane row segment (one 128B swizzle row)
 constexpr int MG_UMMA_K = 32;
-constexpr int MG_THREADS = 256;
+constexpr int MG_EPI_WARPS = 8;  // two per TMEM lane quarter, splitting the column groups
+constexpr int MG_THREADS = 32 * (4 + MG_EPI_WARPS);
 constexpr int MG_A_BYTES = MG_BM * MG_BK;  // 16 KiB: one H limb of one k-atom
 constexpr int MG_ZERO_BYTES = 1024;        // all-zero A operand (one 8-row swizzle atom, aliased by SBO = 0)
 constexpr int MG_MAX_MODULI = 4;
@@ -59,8 +61,9 @@ struct ModGemmParams {
     uint32_t a_stages, b_stages, b_stage_bytes;  // per CTA
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
+    uint32_t dbg;      // timing experiments only (VIPIR_TUNE_MG_DBG): bit0 no D offset, bit1 no epilogue math
     uint32_t moduli[MG_MAX_MODULI];
-    uint32_t c32[MG_MAX_MODULI];      // 2^32 mod q_t
+    uint32_t w[MG_MAX_MODULI][3];     // 2^32, 2^40, 2^48 mod q_t: weights of the three high limb sums
     uint64_t barrett[MG_MAX_MODULI];  // floor(2^64 / q_t)
     const uint32_t* G;                // [P][gcols][M] or nullptr
     uint32_t* out;                    // [P][ncols][M]
@@ -121,12 +124,6 @@ __device__ __forceinline__ uint64_t make_smem_desc_zero(uint32_t saddr) {
     return d;
 }
 
-// (lo + 2^32 * hi) mod q for lo < 2^57, hi < 2^49, q < 2^30: reduce hi, fold with 2^32 mod q
-__device__ __forceinline__ uint64_t mg_fold(uint64_t lo, uint64_t hi, uint32_t q, uint64_t bm, uint32_t c32) {
-    const uint32_t hr = barrett_u64(hi, q, bm);
-    return lo + (uint64_t)hr * c32;  // < 2^57 + 2^60
-}
-
 template <int CG>
 __global__ void __launch_bounds__(MG_THREADS, 1)
 modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, ModGemmParams p) {
@@ -170,7 +167,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
         for (uint32_t a = 0; a < 2; ++a) {
             ptx::mbar_init(&tmem_full[a], 1);
-            ptx::mbar_init(&tmem_empty[a], 4 * CG);
+            ptx::mbar_init(&tmem_empty[a], MG_EPI_WARPS * CG);
         }
         ptx::fence_barrier_init();
     }
@@ -256,7 +253,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
                             for (uint32_t kk = 0; kk < MG_BK / MG_UMMA_K; ++kk) {
                                 const uint64_t koff = (uint64_t)((kk * MG_UMMA_K) >> 4);
-                                ptx::mma_i8<CG>(tacc + i * p.ct, dA + koff, dB + koff, p.idesc,
+                                ptx::mma_i8<CG>(tacc + ((p.dbg & 1) ? 0u : i * p.ct), dA + koff, dB + koff, p.idesc,
                                                 (first && kk == 0) ? 0u : 1u);
                             }
                             if constexpr (CG == 2) ptx::tc_commit_pair(&emptyA[sa], 3);
@@ -273,9 +270,12 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             }
         }
     } else if (warp >= 4) {
-        // ===== epilogue warps: lane quarter = warp % 4 =====
+        // ===== epilogue warps: lane quarter = warp % 4; the two warps of a quarter take alternate
+        // groups of 8 columns =====
         const uint32_t quarter = warp & 3;
+        const uint32_t half = (warp - 4) >> 2;
         const uint32_t g0 = p.ncols - p.gcols;
+        const uint32_t n_groups = (p.dbg & 2) ? 0u : p.ct / 8;  // <= 8
         uint32_t acc_it = 0;
         for (uint32_t u = unit0; u < n_units; u += unit_stride) {
             const uint32_t prob = u / tiles_per_problem, rem = u % tiles_per_problem;
@@ -283,37 +283,68 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const uint32_t row = (mt * CG + rank) * MG_BM + quarter * 32 + lane;
             const bool row_ok = row < p.M;
             const uint32_t t = prob / p.NC;
-            const uint32_t q = p.moduli[t], c32 = p.c32[t];
+            const uint32_t q = p.moduli[t];
+            const uint32_t w4 = p.w[t][0], w5 = p.w[t][1], w6 = p.w[t][2];
             const uint64_t bm = p.barrett[t];
+            const uint32_t* __restrict__ Gp = p.G + ((uint64_t)prob * p.gcols) * p.M + row;
+            uint32_t* __restrict__ Op = p.out + ((uint64_t)prob * p.ncols) * p.M + row;
             for (uint32_t c = 0; c < p.n_chunks; ++c, ++acc_it) {
                 const uint32_t as = acc_it % p.acc_stages;
                 const uint32_t aphase = (acc_it / p.acc_stages) & 1;
-                ptx::mbar_wait(&tmem_full[as], aphase);
-                ptx::tc_fence_after();
-                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols;
-                for (uint32_t g = 0; g < p.ct / 8; ++g) {
-                    uint32_t v[7][8];
+                // The words added to this chunk's sums -- G on the last gcols columns ("(0 | G)") for
+                // chunk 0, the running (reduced) result for later chunks -- do not depend on the
+                // accumulators: all of this warp's are fetched before waiting for the MMAs, so their
+                // global-load latency is paid once per tile and overlaps the products.
+                uint32_t add[4][8];
 #pragma unroll
-                    for (int s = 0; s < 7; ++s) ptx::tmem_ld8(tacc + s * p.ct + g * 8, v[s]);
-                    ptx::tmem_ld_wait();
+                for (int gi = 0; gi < 4; ++gi) {
+                    const uint32_t g = half + 2 * gi;
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const uint32_t col = nt * p.ct + g * 8 + e;
-                        if (col < p.ncols && row_ok) {
-                            // sum_s 2^(8s) S_s, S_s < 2^31 (one K chunk): low four limbs < 2^57, high three < 2^49
-                            const uint64_t lo = (uint64_t)v[0][e] + ((uint64_t)v[1][e] << 8) + ((uint64_t)v[2][e] << 16) +
-                                                ((uint64_t)v[3][e] << 24);
-                            const uint64_t hi = (uint64_t)v[4][e] + ((uint64_t)v[5][e] << 8) + ((uint64_t)v[6][e] << 16);
-                            uint64_t x = mg_fold(lo, hi, q, bm, c32);
-                            uint32_t* dst = p.out + ((uint64_t)prob * p.ncols + col) * p.M + row;
-                            if (c == 0) {
-                                if (col >= g0) x += p.G[((uint64_t)prob * p.gcols + (col - g0)) * p.M + row];  // (0 | G)
-                            } else {
-                                x += *dst;  // earlier K chunks, already reduced
-                            }
-                            *dst = barrett_u64(x, q, bm);
+                        add[gi][e] = 0u;
+                        if (g < n_groups && col < p.ncols && row_ok) {
+                            if (c > 0) add[gi][e] = __ldcg(Op + (uint64_t)col * p.M);
+                            else if (col >= g0) add[gi][e] = __ldg(Gp + (uint64_t)(col - g0) * p.M);
                         }
                     }
+                }
+                ptx::mbar_wait(&tmem_full[as], aphase);
+                ptx::tc_fence_after();
+                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols;
+                // rolled loop: the body always consumes add[0], the prefetched words shift down after
+                // every group (register moves), which keeps the indices compile-time constants
+#pragma unroll 1
+                for (uint32_t g = half; g < n_groups; g += 2) {
+                    {
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            uint32_t v[7][4];
+#pragma unroll
+                            for (int s = 0; s < 7; ++s) ptx::tmem_ld4(tacc + s * p.ct + g * 8 + hh * 4, v[s]);
+                            ptx::tmem_ld_wait();
+#pragma unroll
+                            for (int e4 = 0; e4 < 4; ++e4) {
+                                const int e = hh * 4 + e4;
+                                const uint32_t col = nt * p.ct + g * 8 + e;
+                                if (col < p.ncols && row_ok) {
+                                    // sum_s 2^(8s) S_s with S_s < 2^31 (one K chunk).  The low four limb
+                                    // sums are combined with shifts (< 2^57); the high three are weighted
+                                    // by 2^(8s) mod q < 2^30 (each product < 2^61), so the total stays
+                                    // below 2^63 and ONE Barrett reduction per output word remains.
+                                    uint64_t x = (uint64_t)v[0][e4] + ((uint64_t)v[1][e4] << 8) +
+                                                 ((uint64_t)v[2][e4] << 16) + ((uint64_t)v[3][e4] << 24);
+                                    x += (uint64_t)v[4][e4] * w4 + (uint64_t)v[5][e4] * w5 + (uint64_t)v[6][e4] * w6;
+                                    x += add[0][e];
+                                    Op[(uint64_t)col * p.M] = barrett_u64(x, q, bm);
+                                }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int gi = 0; gi < 3; ++gi)
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) add[gi][e] = add[gi + 1][e];
                 }
                 ptx::tc_fence_before();
                 __syncwarp();
