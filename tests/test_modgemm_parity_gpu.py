@@ -209,3 +209,57 @@ def test_modgemm_parts_equal_whole_and_errors():
         d_O = torch.zeros((1, 1, 2, 8), dtype=torch.int32, device="cuda")
         with pytest.raises(vipir.VipirError):
             vipir.modgemm_products(plan.handle, None, d_O)
+
+
+# ---- the paper's full shape (64 GiB DB, N = 2^12, D_r = 2^8, n = 1280, #RNS = 3) --------
+# T*NC = 12288 problems of 256 x 2B x 1280; H is 15 GiB ("H occupies 15GiB of memory space", :222).
+# Compared on sampled problems the oracle recomputes in full from the host generator's words, plus a
+# row-sum identity over ALL problems that holds at any size (linearity):
+#     sum_m Out[p][j][m] = sum_k (sum_m H[p][m][k]) * C[p][j][k] + sum_m G[p][j-g0][m]      (mod q_t)
+# with the sums taken by plain torch reductions that share nothing with libvipir.
+
+FULL_T, FULL_NC, FULL_M, FULL_K = 3, 4096, 256, 1280
+
+
+@pytest.mark.parametrize("B", [1, 32])
+def test_modgemm_paper_shape_sampled_problems_and_row_sums(B):
+    import torch
+    from paper_2606_11536_b200.inputs import device
+    ensure_built()
+    torch.cuda.empty_cache()
+    moduli = P29
+    T, NC, M, K = FULL_T, FULL_NC, FULL_M, FULL_K
+    ncols, gcols = 2 * B, B
+    g0 = ncols - gcols
+    d_H = device.modgemm_operand(0, gen.STREAM_MG_H, moduli, NC, M * K).view(T, NC, M, K)
+    d_C = device.modgemm_operand(0, gen.STREAM_MG_C, moduli, NC, ncols * K).view(T, NC, ncols, K)
+    d_G = device.modgemm_operand(0, gen.STREAM_MG_G, moduli, NC, gcols * M).view(T, NC, gcols, M)
+    d_O = torch.full((T, NC, ncols, M), -1, dtype=torch.int32, device="cuda")
+    with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli) as plan:
+        plan.set_h(d_H)
+        plan(d_C, d_G, d_O)  # the launch configuration bench.py times (the planner's own choice)
+        torch.cuda.synchronize()
+
+    # (1) sampled problems, every output word
+    cs = sorted(set([0, 1, NC // 2, NC - 1] + np.random.default_rng(B).integers(0, NC, size=6).tolist()))
+    for c in cs:
+        H = gen.modgemm_operand(0, gen.STREAM_MG_H, moduli, NC, M * K, c0=c, nc=1).reshape(T, 1, M, K)
+        C = gen.modgemm_operand(0, gen.STREAM_MG_C, moduli, NC, ncols * K, c0=c, nc=1).reshape(T, 1, ncols, K)
+        G = gen.modgemm_operand(0, gen.STREAM_MG_G, moduli, NC, gcols * M, c0=c, nc=1).reshape(T, 1, gcols, M)
+        want = oracle.modgemm(H, C, G, moduli, nthreads=NT)
+        got = d_O[:, c:c + 1].cpu().numpy().view(np.uint32)
+        assert_same(got, want)
+
+    # (2) row-sum identity over all problems; canonical range of every word
+    for t, q in enumerate(moduli):
+        assert int(d_O[t].max()) < q and int(d_O[t].min()) >= 0
+        for c0 in range(0, NC, 512):
+            sl = slice(c0, c0 + 512)
+            hs = d_H[t, sl].to(torch.int64).sum(dim=1) % q                       # [nc][K], each < q < 2^29
+            terms = (hs[:, None, :] * d_C[t, sl].to(torch.int64)) % q            # products < 2^58
+            want = terms.sum(dim=2)                                              # < 1280 * 2^29
+            want[:, g0:] += d_G[t, sl].to(torch.int64).sum(dim=2)
+            got = d_O[t, sl].to(torch.int64).sum(dim=2)
+            assert torch.equal(got % q, want % q), f"row-sum identity fails: modulus {t}, problems {c0}.."
+    del d_H, d_C, d_G, d_O
+    torch.cuda.empty_cache()
