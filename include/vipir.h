@@ -85,7 +85,7 @@ typedef struct {
     uint32_t tile_queries;    /* query vectors per N tile (MMA regimes) */
     uint32_t tile_cols;       /* accumulator columns per tile = tile_queries * LC */
     uint32_t mma_n;           /* N of one tcgen05.mma */
-    uint32_t m_tiles, n_tiles;
+    uint32_t m_tiles, n_tiles; /* a work unit = one (M tile, N tile); units x n_chunks work items are dealt to the CTAs */
     uint32_t stages;          /* shared-memory ring depth */
     uint32_t smem_bytes;      /* dynamic shared memory per CTA */
     uint32_t grid;            /* CTAs launched by the main kernel */
@@ -94,6 +94,7 @@ typedef struct {
     void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
     uint32_t modswitch_bits;  /* fused output modulus switch in effect (0 = off) */
     uint32_t db_signed;       /* 1 if the DB elements are read as two's-complement int8 (vipir_plan_set_db_signed) */
+    uint32_t m_sub;           /* MMA regimes: 128-row DB sub-tiles per CTA and tile (rows per tile = 128 * CTAs * m_sub) */
 } vipir_info;
 
 /*

@@ -25,6 +25,23 @@
 // accumulators are drained after every chunk.  With CG = 2 a pair of CTAs (one cluster of 2
 // SMs) runs cta_group::2 MMAs: M = 256 rows per pair, each CTA stages its own 128 DB rows and
 // HALF of the limb-plane tile, halving shared-memory fill and read traffic per SM.
+//
+// M sub-tiles (msub = 1, 2, 4): while the product is HBM-bound what limits it is the L2 -> SM
+// fill (DB bytes + the limb tile re-read by every M tile), so a CTA keeps msub 128-row DB
+// sub-tiles per k-atom against ONE limb-tile box: msub accumulators side by side in TMEM, the
+// limb-plane traffic per DB byte divided by msub.
+//
+// Work distribution.  A work item is (unit = (M tile, N tile), K chunk).  Groups (a CTA, or a
+// CTA pair) take whole units round-robin for the full rounds -- so that the sibling N tiles of
+// one M tile run at the same time on neighbouring groups and share the DB tile through L2 --
+// and the units of the last, partial round are dealt out chunk by chunk in contiguous item
+// ranges, which removes the wave-quantisation loss (e.g. 256 units on 74 pairs: 3.5 rounds
+// instead of 4).  A unit split between two groups is accumulated through the answer buffer
+// (chunk 0 stores, later chunks add): the later group waits on a per-unit arrival counter in
+// global memory before its first read-modify-write.  Group ids are tickets drawn from an atomic
+// counter, a group only ever waits for lower tickets, and every group works through its
+// producing items (the tail of its range) first, so the waits cannot deadlock whatever order the
+// hardware starts the CTAs in; the last group to finish resets the counters for the next launch.
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -56,6 +73,10 @@ struct GemmParams {
     uint32_t stages;
     uint32_t stage_bytes;    // per CTA = katoms * atom_bytes
     uint32_t tmem_cols, acc_stages;
+    uint32_t msub;           // 128-row DB sub-tiles per CTA and unit (1, 2 or 4): rows per unit = 128 * CG * msub
+    uint32_t split;          // deal the last, partial round out chunk by chunk (1) or unit by unit (0)
+    uint32_t n_groups;       // CTAs (CG = 1) or CTA pairs (CG = 2) launched
+    uint32_t* sync;          // [0] ticket, [1] groups finished, [2 + i] epilogue-warp arrivals of leftover unit i
     uint32_t idesc;
     uint32_t ms_bits;        // fused modulus switch 2^32 -> 2^ms_bits of the answer (0 = off; q = 2^32 only)
     uint32_t db_signed;      // DB bytes are s8 (A format s8 in idesc): the s32 accumulators may be negative
@@ -84,6 +105,72 @@ __device__ __forceinline__ uint32_t barrett_u64(uint64_t x, uint32_t p, uint64_t
     return (uint32_t)r;
 }
 
+// ---- work distribution (see the header comment) ------------------------------------------------
+// Group g of G: units  r*G + g  for the full rounds r < n_units / G  (all chunks), then the item range
+// [g*I/G, (g+1)*I/G) of the I = L*nc leftover items (L = n_units mod G units, unit-major), visited in
+// the order  tail (chunks [0, c) of the range's last unit)  ->  whole units  ->  head (chunks
+// [c0, c1) of the range's first unit, whose earlier chunks belong to group g-1 or before).
+struct WorkPlan {
+    uint32_t g, G, nc, full_rounds, u_base;
+    uint32_t has_tail, tail_u, tail_c1;
+    uint32_t mid0, mid1;
+    uint32_t has_head, head_u, head_c0, head_c1;
+};
+
+__device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t G, uint32_t n_units, uint32_t nc,
+                                                   uint32_t split) {
+    WorkPlan w;
+    w.g = g; w.G = G; w.nc = nc;
+    w.full_rounds = n_units / G;
+    w.u_base = w.full_rounds * G;
+    const uint32_t L = n_units - w.u_base;
+    if (!split) {  // leftover units whole, one per group
+        w.has_head = w.has_tail = 0;
+        w.head_u = w.head_c0 = w.head_c1 = w.tail_u = w.tail_c1 = 0;
+        w.mid0 = w.u_base + (g < L ? g : L);
+        w.mid1 = w.u_base + (g < L ? g + 1 : L);
+        return w;
+    }
+    const uint64_t I = (uint64_t)L * nc;
+    const uint32_t b = (uint32_t)((uint64_t)g * I / G), e = (uint32_t)((uint64_t)(g + 1) * I / G);
+    const uint32_t ub = b / nc, cb = b % nc, ue = e / nc, ce = e % nc;
+    w.has_head = (e > b && cb != 0) ? 1u : 0u;
+    w.head_u = w.u_base + ub;
+    w.head_c0 = cb;
+    w.head_c1 = (ue == ub) ? ce : nc;
+    const uint32_t m0 = cb ? ub + 1 : ub;
+    w.mid0 = w.u_base + m0;
+    w.mid1 = w.u_base + (ue > m0 ? ue : m0);
+    w.has_tail = (e > b && ce != 0 && !(cb != 0 && ue == ub)) ? 1u : 0u;
+    w.tail_u = w.u_base + ue;
+    w.tail_c1 = ce;
+    return w;
+}
+
+// f(unit, chunk, must_wait): must_wait marks the first item of a head segment -- the chunks before
+// it were (or are being) accumulated into the answer by another group.
+template <class F>
+__device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f) {
+    // four segments, one loop nest (a single copy of the caller's body)
+#pragma unroll 1
+    for (uint32_t seg = 0; seg < 4; ++seg) {
+        uint32_t u_lo, u_hi, u_step = 1, c_lo = 0, c_hi = w.nc;
+        if (seg == 0) {  // full rounds
+            u_lo = w.g; u_hi = w.u_base; u_step = w.G;
+        } else if (seg == 1) {  // tail of the leftover range: produces chunks another group continues
+            u_lo = w.tail_u; u_hi = w.tail_u + w.has_tail; c_hi = w.tail_c1;
+        } else if (seg == 2) {  // whole leftover units
+            u_lo = w.mid0; u_hi = w.mid1;
+        } else {  // head: continues a unit another group started
+            u_lo = w.head_u; u_hi = w.head_u + w.has_head; c_lo = w.head_c0; c_hi = w.head_c1;
+        }
+#pragma unroll 1
+        for (uint32_t u = u_lo; u < u_hi; u += u_step)
+#pragma unroll 1
+            for (uint32_t c = c_lo; c < c_hi; ++c) f(u, c, seg == 3 && c == c_lo);
+    }
+}
+
 template <int CG, int LC, bool PRIME>
 __global__ void __launch_bounds__(GM_THREADS, 1)
 gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, GemmParams p) {
@@ -94,17 +181,24 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     uint64_t* tmem_full = empty + p.stages;   // [2]
     uint64_t* tmem_empty = tmem_full + 2;     // [2]
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    uint32_t* ticket_ptr = tmem_ptr + 1;
+    uint32_t* last_ptr = tmem_ptr + 2;
 
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
-    const uint32_t unit0 = (CG == 2) ? ptx::cluster_id_x() : blockIdx.x;
-    const uint32_t unit_stride = (CG == 2) ? ptx::num_clusters_x() : gridDim.x;
     const uint32_t n_units = p.m_tiles * p.n_tiles;
+    const uint32_t acc_cols = p.msub * p.bn;  // TMEM columns of one accumulator stage
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmA);
         ptx::prefetch_tmap(&tmB);
+        // group id = ticket: a group only ever waits for groups that drew a lower ticket, i.e. that
+        // are already running
+        if (rank == 0) {
+            const uint32_t t = atomicAdd(p.sync, 1u);
+            *ticket_ptr = p.split ? t : ((CG == 2) ? ptx::cluster_id_x() : blockIdx.x);
+        }
     }
     if (warp == 1 && lane == 0) {
         for (uint32_t s = 0; s < p.stages; ++s) {
@@ -124,127 +218,162 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     ptx::tc_fence_before();
     if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tmem_base = *tmem_ptr;
+    // values read back from shared memory are the same in every lane: say so (shfl from lane 0), so
+    // that the single-issuer loops below run on the uniform datapath instead of per-lane registers
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+    // the pair's ticket lives in the leader's shared memory (the leader outlives this read: the
+    // teardown ends with a cluster barrier)
+    const uint32_t ticket = __shfl_sync(
+        0xffffffffu, (CG == 2 && rank == 1) ? ptx::ld_shared_cluster_u32(ticket_ptr, 0) : *ticket_ptr, 0);
+    const WorkPlan work = make_work_plan(ticket, p.n_groups, n_units, p.n_chunks, p.split);
 
     if (warp == 0) {
-        // ===== TMA producer =====
-        if (lane == 0) {
+        // ===== TMA producer: the whole warp runs the (warp-uniform) loop, one elected lane issues =====
+        {
             uint32_t stage = 0, phase = 0;
             const uint32_t b_rows = p.ni_cols / CG;  // limb-plane rows this CTA stages per instruction
             const uint32_t b_bytes = b_rows * GM_BK;
-            for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+            // the DB is streamed once (evict_first); with several N tiles the sibling tiles, which
+            // run alongside on neighbouring clusters, re-read it from L2, so it stays evict_normal
+            // (ncu: marking the last sibling evict_first raised DRAM reads from 5.6 to 8.0 GB on C4)
+            const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+            for_each_item(work, [&](uint32_t u, uint32_t c, bool) {
                 const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
-                // the DB is streamed once (evict_first); with several N tiles the sibling tiles, which
-                // run alongside on neighbouring clusters, re-read it from L2, so it stays evict_normal
-                // (ncu: marking the last sibling evict_first raised DRAM reads from 5.6 to 8.0 GB on C4)
-                const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
-                const int32_t row0 = (int32_t)((mt * CG + rank) * GM_BM);
-                for (uint32_t c = 0; c < p.n_chunks; ++c) {
-                    const uint32_t ks_begin = c * p.ksteps_per_chunk;
-                    const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
-                    // a stage never straddles a chunk: the last stage of a chunk may hold fewer atoms
-                    for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
-                        const uint32_t na = min(p.katoms, ks_end - ks0);
-                        ptx::mbar_wait(&empty[stage], phase ^ 1);
-                        uint8_t* sbase = smem + (size_t)stage * p.stage_bytes;
-                        uint32_t bar = 0;
-                        if constexpr (CG == 1) {
-                            ptx::mbar_arrive_expect_tx(&full[stage], na * p.atom_bytes);
-                        } else {
-                            // both CTAs' bytes are counted on the leader's barrier
-                            if (rank == 0) ptx::mbar_arrive_expect_tx(&full[stage], 2 * na * p.atom_bytes);
-                            bar = ptx::mapa(ptx::smem_u32(&full[stage]), 0);
-                        }
-                        for (uint32_t a = 0; a < na; ++a) {
-                            uint8_t* sA = sbase + a * p.atom_bytes;
-                            uint8_t* sB = sA + GM_A_BYTES;
-                            const int32_t k0 = (int32_t)((ks0 + a) * GM_BK);
-                            if constexpr (CG == 1) {
-                                ptx::tma_load_2d(sA, &tmA, &full[stage], k0, row0, hintA);
-                                for (uint32_t j = 0; j < p.n_instr; ++j)
-                                    ptx::tma_load_2d(sB + j * b_bytes, &tmB, &full[stage], k0,
-                                                     (int32_t)(nt * p.bn + j * p.ni_cols), ptx::kEvictLast);
-                            } else {
-                                ptx::tma_load_2d_pair(sA, &tmA, bar, k0, row0, hintA);
-                                for (uint32_t j = 0; j < p.n_instr; ++j)
-                                    ptx::tma_load_2d_pair(sB + j * b_bytes, &tmB, bar, k0,
-                                                          (int32_t)(nt * p.bn + j * p.ni_cols + rank * b_rows),
-                                                          ptx::kEvictLast);
-                            }
-                        }
-                        if (++stage == p.stages) { stage = 0; phase ^= 1; }
+                // sub-tile j of the unit = rows [(mt*msub + j) * 128*CG, +128*CG); this CTA's 128 of them
+                const int32_t row0 = (int32_t)((mt * p.msub * CG + rank) * GM_BM);
+                const uint32_t ks_begin = c * p.ksteps_per_chunk;
+                const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
+                // a stage never straddles a chunk: the last stage of a chunk may hold fewer atoms
+                for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
+                    const uint32_t na = min(p.katoms, ks_end - ks0);
+                    ptx::mbar_wait(&empty[stage], phase ^ 1);
+                    __syncwarp();
+                    if (ptx::elect_one()) {
+                    uint8_t* sbase = smem + (size_t)stage * p.stage_bytes;
+                    uint32_t bar = 0;
+                    if constexpr (CG == 1) {
+                        ptx::mbar_arrive_expect_tx(&full[stage], na * p.atom_bytes);
+                    } else {
+                        // both CTAs' bytes are counted on the leader's barrier
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(&full[stage], 2 * na * p.atom_bytes);
+                        bar = ptx::mapa(ptx::smem_u32(&full[stage]), 0);
                     }
+                    for (uint32_t a = 0; a < na; ++a) {
+                        uint8_t* sA = sbase + a * p.atom_bytes;
+                        uint8_t* sB = sA + p.msub * GM_A_BYTES;
+                        const int32_t k0 = (int32_t)((ks0 + a) * GM_BK);
+                        if constexpr (CG == 1) {
+                            for (uint32_t j = 0; j < p.msub; ++j)
+                                ptx::tma_load_2d(sA + j * GM_A_BYTES, &tmA, &full[stage], k0,
+                                                 row0 + (int32_t)(j * GM_BM), hintA);
+                            for (uint32_t j = 0; j < p.n_instr; ++j)
+                                ptx::tma_load_2d(sB + j * b_bytes, &tmB, &full[stage], k0,
+                                                 (int32_t)(nt * p.bn + j * p.ni_cols), ptx::kEvictLast);
+                        } else {
+                            for (uint32_t j = 0; j < p.msub; ++j)
+                                ptx::tma_load_2d_pair(sA + j * GM_A_BYTES, &tmA, bar, k0,
+                                                      row0 + (int32_t)(j * 2 * GM_BM), hintA);
+                            for (uint32_t j = 0; j < p.n_instr; ++j)
+                                ptx::tma_load_2d_pair(sB + j * b_bytes, &tmB, bar, k0,
+                                                      (int32_t)(nt * p.bn + j * p.ni_cols + rank * b_rows),
+                                                      ptx::kEvictLast);
+                        }
+                    }
+                    }
+                    __syncwarp();
+                    if (++stage == p.stages) { stage = 0; phase ^= 1; }
                 }
-            }
+            });
         }
     } else if (warp == 1) {
         // ===== MMA issuer (leader CTA of the pair only) =====
-        if (rank == 0 && lane == 0) {
+        // the whole warp runs the (warp-uniform) loop; one elected lane -- the same one every time, so
+        // that tcgen05.commit tracks the MMAs it issued -- issues
+        if (rank == 0) {
             uint32_t stage = 0, phase = 0, acc_it = 0;
             const uint32_t b_bytes = (p.ni_cols / CG) * GM_BK;
-            for (uint32_t u = unit0; u < n_units; u += unit_stride) {
-                for (uint32_t c = 0; c < p.n_chunks; ++c, ++acc_it) {
-                    const uint32_t as = acc_it % p.acc_stages;
-                    const uint32_t aphase = (acc_it / p.acc_stages) & 1;
-                    if constexpr (CG == 2) ptx::mbar_wait_cluster(&tmem_empty[as], aphase ^ 1);
-                    else ptx::mbar_wait(&tmem_empty[as], aphase ^ 1);
+            for_each_item(work, [&](uint32_t, uint32_t c, bool) {
+                const uint32_t as = acc_it % p.acc_stages;
+                const uint32_t aphase = (acc_it / p.acc_stages) & 1;
+                ++acc_it;
+                if constexpr (CG == 2) ptx::mbar_wait_cluster(&tmem_empty[as], aphase ^ 1);
+                else ptx::mbar_wait(&tmem_empty[as], aphase ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t ks_begin = c * p.ksteps_per_chunk;
+                const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
+                const uint32_t tacc = tmem_base + as * acc_cols;
+                for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
+                    const uint32_t na = min(p.katoms, ks_end - ks0);
+                    ptx::mbar_wait(&full[stage], phase);
                     ptx::tc_fence_after();
-                    const uint32_t ks_begin = c * p.ksteps_per_chunk;
-                    const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
-                    const uint32_t tacc = tmem_base + as * p.bn;
-                    for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
-                        const uint32_t na = min(p.katoms, ks_end - ks0);
-                        ptx::mbar_wait(&full[stage], phase);
-                        ptx::tc_fence_after();
-                        const uint32_t sbase = ptx::smem_u32(smem + (size_t)stage * p.stage_bytes);
-                        for (uint32_t a = 0; a < na; ++a) {
-                            const uint32_t sA = sbase + a * p.atom_bytes;
-                            const uint32_t sB = sA + GM_A_BYTES;
-                            const uint64_t dA = make_smem_desc(sA);
+                    __syncwarp();
+                    if (ptx::elect_one()) {
+                    const uint32_t sbase = ptx::smem_u32(smem + (size_t)stage * p.stage_bytes);
+                    for (uint32_t a = 0; a < na; ++a) {
+                        const uint32_t sA = sbase + a * p.atom_bytes;
+                        const uint32_t sB = sA + p.msub * GM_A_BYTES;
+                        const uint32_t accumulate = (ks0 + a > ks_begin) ? 1u : 0u;
+                        for (uint32_t m = 0; m < p.msub; ++m) {
+                            const uint64_t dA = make_smem_desc(sA + m * GM_A_BYTES);
                             for (uint32_t j = 0; j < p.n_instr; ++j) {
                                 const uint64_t dB = make_smem_desc(sB + j * b_bytes);
 #pragma unroll
                                 for (uint32_t kk = 0; kk < GM_BK / GM_UMMA_K; ++kk) {
                                     // advancing K inside the swizzle atom = adding the byte offset >> 4
                                     const uint64_t koff = (uint64_t)((kk * GM_UMMA_K) >> 4);
-                                    ptx::mma_i8<CG>(tacc + j * p.ni_cols, dA + koff, dB + koff, p.idesc,
-                                                    (ks0 + a > ks_begin || kk > 0) ? 1u : 0u);
+                                    ptx::mma_i8<CG>(tacc + m * p.bn + j * p.ni_cols, dA + koff, dB + koff, p.idesc,
+                                                    (accumulate || kk > 0) ? 1u : 0u);
                                 }
                             }
                         }
-                        // release the smem slot once these MMAs have read it
-                        if constexpr (CG == 2) ptx::tc_commit_pair(&empty[stage], 3);
-                        else ptx::tc_commit(&empty[stage]);
-                        if (++stage == p.stages) { stage = 0; phase ^= 1; }
                     }
+                    // release the smem slot once these MMAs have read it
+                    if constexpr (CG == 2) ptx::tc_commit_pair(&empty[stage], 3);
+                    else ptx::tc_commit(&empty[stage]);
                     // accumulators of this chunk complete -> epilogue
-                    if constexpr (CG == 2) ptx::tc_commit_pair(&tmem_full[as], 3);
-                    else ptx::tc_commit(&tmem_full[as]);
+                    if (ks0 + na >= ks_end) {
+                        if constexpr (CG == 2) ptx::tc_commit_pair(&tmem_full[as], 3);
+                        else ptx::tc_commit(&tmem_full[as]);
+                    }
+                    }
+                    __syncwarp();
+                    if (++stage == p.stages) { stage = 0; phase ^= 1; }
                 }
-            }
+            });
         }
     } else if (warp >= 4) {
         // ===== epilogue warps: lane quarter = warp % 4 =====
         const uint32_t quarter = warp & 3;
         uint32_t acc_it = 0;
-        for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+        for_each_item(work, [&](uint32_t u, uint32_t c, bool must_wait) {
             const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
-            const uint64_t row = (uint64_t)(mt * CG + rank) * GM_BM + quarter * 32 + lane;
-            const bool row_ok = row < p.rows;
-            for (uint32_t c = 0; c < p.n_chunks; ++c, ++acc_it) {
-                const uint32_t as = acc_it % p.acc_stages;
-                const uint32_t aphase = (acc_it / p.acc_stages) & 1;
-                ptx::mbar_wait(&tmem_full[as], aphase);
-                ptx::tc_fence_after();
-                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * p.bn;
-                // later chunks add to what chunk 0 stored: a fire-and-forget red.add for q = 2^32; for
-                // primes the old words are fetched eight steps (32 query vectors) at a time so that
-                // one global-load latency is paid per batch, not per step
-                // with the fused modulus switch (q = 2^32 only) the LAST chunk needs the running sum back
-                // to round it: same batched prefetch, once per tile
-                constexpr uint32_t kPf = 8;
-                const bool ms_final = !PRIME && p.ms_bits != 0 && c + 1 == p.n_chunks;
-                const bool need_old = c > 0 && (PRIME || ms_final);
+            const uint32_t as = acc_it % p.acc_stages;
+            const uint32_t aphase = (acc_it / p.acc_stages) & 1;
+            ++acc_it;
+            ptx::mbar_wait(&tmem_full[as], aphase);
+            ptx::tc_fence_after();
+            if (must_wait) {
+                // chunks [0, c) of this unit belong to another group: all of its (4 * CG) epilogue
+                // warps must have stored them before this read-modify-write (see "Work distribution")
+                const uint32_t* cnt = p.sync + 2 + (u - work.u_base);
+                const uint32_t want = c * 4 * CG;
+                const long long t0 = clock64();
+                while (ptx::ld_acquire_gpu(cnt) < want) {
+                    if (clock64() - t0 > (20ll << 30)) __trap();  // ~10 s: never in a correct run
+                }
+            }
+            // later chunks add to what chunk 0 stored: a fire-and-forget red.add for q = 2^32; for
+            // primes the old words are fetched eight steps (32 query vectors) at a time so that
+            // one global-load latency is paid per batch, not per step
+            // with the fused modulus switch (q = 2^32 only) the LAST chunk needs the running sum back
+            // to round it: same batched prefetch, once per tile
+            constexpr uint32_t kPf = 8;
+            const bool ms_final = !PRIME && p.ms_bits != 0 && c + 1 == p.n_chunks;
+            const bool need_old = c > 0 && (PRIME || ms_final);
+            for (uint32_t m = 0; m < p.msub; ++m) {
+                const uint64_t row = (uint64_t)((mt * p.msub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
+                const bool row_ok = row < p.rows;
+                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols + m * p.bn;
                 for (uint32_t g0 = 0; g0 < p.qt / 4; g0 += kPf) {
                     uint32_t old[4 * kPf];
                     if (need_old) {
@@ -309,15 +438,18 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         }
                     }
                 }
-                // accumulator stage drained
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) {
-                    if constexpr (CG == 2) ptx::mbar_arrive_cluster(&tmem_empty[as], 0);
-                    else ptx::mbar_arrive(&tmem_empty[as]);
-                }
             }
-        }
+            // accumulator stage drained
+            ptx::tc_fence_before();
+            if (u >= work.u_base) __threadfence();  // this lane's answer words, before the arrival below
+            __syncwarp();
+            if (lane == 0) {
+                if constexpr (CG == 2) ptx::mbar_arrive_cluster(&tmem_empty[as], 0);
+                else ptx::mbar_arrive(&tmem_empty[as]);
+                // units of the leftover round may be shared with another group: count this warp in
+                if (u >= work.u_base) ptx::red_release_gpu_add(p.sync + 2 + (u - work.u_base), 1u);
+            }
+        });
     }
 
     // ===== teardown =====
@@ -326,6 +458,18 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if (warp == 2) {
         ptx::tc_fence_after();
         ptx::tmem_dealloc<CG>(tmem_base, p.tmem_cols);
+    }
+    // the last group to finish leaves the ticket and the arrival counters at zero for the next launch
+    if (rank == 0) {
+        if (threadIdx.x == 0) {
+            __threadfence();
+            *last_ptr = (atomicAdd(p.sync + 1, 1u) == p.n_groups - 1) ? 1u : 0u;
+        }
+        __syncthreads();
+        if (*last_ptr) {
+            __threadfence();
+            for (uint32_t i = threadIdx.x; i < 2 + p.n_groups; i += GM_THREADS) p.sync[i] = 0u;
+        }
     }
 }
 

@@ -92,6 +92,7 @@ struct vipir_plan {
     // workspace
     uint8_t* d_planes;
     uint64_t planes_bytes;
+    uint32_t* d_sync;  // MMA regimes: ticket, finished-groups count, per-leftover-unit arrival counters
     // host-call staging
     uint32_t* d_q_stage;
     uint32_t* d_a_stage;
@@ -181,14 +182,31 @@ int plan_gemm(vipir_plan* p, int cg) {
     g.qt = qt;
     g.bn = bn;
     g.n_tiles = ceil_div(p->nq, qt);
-    g.m_tiles = (uint32_t)((p->rows + 128ull * cg - 1) / (128ull * cg));
     g.n_instr = (bn > 256) ? 2u : 1u;
     g.ni_cols = bn / g.n_instr;
     g.total_ksteps = (uint32_t)((p->kbytes + vipir::GM_BK - 1) / vipir::GM_BK);
     const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
     g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
-    g.atom_bytes = vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
+    const uint32_t max_groups = (uint32_t)p->num_sms / cg;
+    // M sub-tiles per CTA (gemm_i8_tcgen05.cuh): while the product is HBM-bound every DB byte drags
+    // bn / (128 * cg * msub) limb-plane bytes through L2 -> SM with it, and that fill (~8 TB/s on the
+    // whole chip) is what caps the scan; so take the most sub-tiles that keep two accumulator stages
+    // in TMEM, three pipeline stages in shared memory and >= 2 work items per group.
+    uint32_t msub = 1;
+    for (uint32_t cand = 4; cand > 1; cand >>= 1) {
+        const uint64_t units = (p->rows + 128ull * cg * cand - 1) / (128ull * cg * cand) * g.n_tiles;
+        const uint32_t atom = cand * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
+        if (2 * cand * bn <= 512 && 3 * atom <= kMaxSmem - 1280 && units * g.n_chunks >= 2ull * max_groups) {
+            msub = cand;
+            break;
+        }
+    }
+    const uint32_t msub_force = tune_env("VIPIR_TUNE_MSUB", 0);
+    if ((msub_force == 1 || msub_force == 2 || msub_force == 4) && msub_force * bn <= 512) msub = msub_force;
+    g.msub = msub;
+    g.m_tiles = (uint32_t)((p->rows + 128ull * cg * msub - 1) / (128ull * cg * msub));
+    g.atom_bytes = msub * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
     const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
     // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes"); VIPIR_TUNE_* override
     // measured on B200 (profiles/r01_tuning.md): several k-atoms per stage (longer contiguous DB
@@ -207,8 +225,8 @@ int plan_gemm(vipir_plan* p, int cg) {
     if (want >= 2 && want < stages) stages = want;
     if (stages < 2) return VIPIR_ERR_UNSUPPORTED;
     g.stages = stages;
-    g.acc_stages = (2 * bn <= 512) ? 2u : 1u;
-    uint32_t cols_needed = g.acc_stages * bn, tc = 32;
+    g.acc_stages = (2 * msub * bn <= 512) ? 2u : 1u;
+    uint32_t cols_needed = g.acc_stages * msub * bn, tc = 32;
     while (tc < cols_needed) tc <<= 1;
     g.tmem_cols = tc;
     g.idesc = (2u << 4) /* D = s32 */ | (0u << 7) /* A = u8 */ | (0u << 10) /* B = u8 */ |
@@ -219,9 +237,22 @@ int plan_gemm(vipir_plan* p, int cg) {
         g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / p->moduli[t]);
     }
     p->smem_bytes = stages * g.stage_bytes + overhead;
-    const uint32_t units = g.m_tiles * g.n_tiles;
-    const uint32_t max_units = (uint32_t)p->num_sms / cg;
-    p->grid = (units < max_units ? units : max_units) * cg;
+    // groups: one per SM (pair); fewer only when there are fewer work items (unit, K chunk) than that
+    const uint64_t items = (uint64_t)g.m_tiles * g.n_tiles * g.n_chunks;
+    g.split = tune_env("VIPIR_TUNE_SPLIT", 1);
+    const uint64_t n_units64 = (uint64_t)g.m_tiles * g.n_tiles;
+    g.n_groups = (uint32_t)(items < max_groups ? items : max_groups);
+    if (!g.split && n_units64 < g.n_groups) g.n_groups = (uint32_t)n_units64;
+    p->grid = g.n_groups * cg;
+    if (!p->d_sync) {
+        const size_t sync_bytes = (2 + (size_t)max_groups) * sizeof(uint32_t);
+        if (cudaMalloc(&p->d_sync, sync_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return VIPIR_ERR_ALLOC;
+        }
+        CK(cudaMemset(p->d_sync, 0, sync_bytes));
+    }
+    g.sync = p->d_sync;
     // limb-plane tensor map: [nq*LC][K'] bytes, box 128 B x (ni_cols / cg) rows, 128B swizzle
     return make_tmap_2d(&p->tm_planes, p->d_planes, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes,
                         (uint64_t)p->nq * lc, p->kbytes, vipir::GM_BK, g.ni_cols / cg, CU_TENSOR_MAP_SWIZZLE_128B);
@@ -481,6 +512,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
         o->m_tiles = p->gm.m_tiles;
         o->n_tiles = p->gm.n_tiles;
         o->stages = p->gm.stages;
+        o->m_sub = p->gm.msub;
     } else if (p->regime == VIPIR_REGIME_GEMV) {
         o->n_chunks = 1;
         o->m_tiles = p->gv.n_blocks;
@@ -493,6 +525,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
 void vipir_destroy(vipir_plan* p) {
     if (!p) return;
     if (p->d_planes) cudaFree(p->d_planes);
+    if (p->d_sync) cudaFree(p->d_sync);
     if (p->d_q_stage) cudaFree(p->d_q_stage);
     if (p->d_a_stage) cudaFree(p->d_a_stage);
     delete p;

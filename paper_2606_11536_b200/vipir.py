@@ -43,7 +43,7 @@ class Info(ctypes.Structure):
         ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32), ("n_tiles", ctypes.c_uint32),
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
         ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
-        ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32),
+        ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32), ("m_sub", ctypes.c_uint32),
     ]
 
     def as_dict(self):

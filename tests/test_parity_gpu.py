@@ -140,6 +140,64 @@ def test_mma_large_batch_two_n_tiles(regime):
     assert_same(got, oracle.dbmul(D, Q, None, nthreads=NT))
 
 
+# ---- M sub-tiles and chunk-granular work distribution (gemm_i8_tcgen05.cuh header) ---------------
+
+@pytest.mark.parametrize("regime", [M1, M2])
+@pytest.mark.parametrize("msub", [2, 4])
+@pytest.mark.parametrize("moduli,bits", [(None, 0), (None, 18), (PRIMES, 0)])
+def test_mma_m_subtiles(regime, msub, moduli, bits, monkeypatch):
+    # rows: several (128 * CG * msub)-row units + a ragged tail that leaves whole sub-tiles empty;
+    # K: 3 chunks, so units are split between groups and accumulated through the answer buffer
+    monkeypatch.setenv("VIPIR_TUNE_MSUB", str(msub))
+    rows, cols, batch = 128 * 2 * msub * 2 + 128 + 37, 32768 * 2 + 2064, 6
+    D, Q = make(300 + msub, rows, cols, batch, 8, moduli)
+    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=bits)
+    assert info["m_sub"] == msub and info["n_chunks"] == 3
+    want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+    if bits:
+        want = oracle.modswitch(want, bits)
+    assert_same(got, want)
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+def test_mma_m_subtiles_permutation_probe(regime, monkeypatch):
+    monkeypatch.setenv("VIPIR_TUNE_MSUB", "4")
+    rows, cols, batch = 128 * 2 * 4 * 2, 512, 8
+    rng = np.random.default_rng(5)
+    perm = rng.integers(0, cols, size=rows)
+    D = np.zeros((rows, cols), dtype=np.uint8)
+    D[np.arange(rows), perm] = 1
+    Q = np.stack([(np.arange(cols, dtype=np.uint64) + 1) * (b + 1) * 0x01010101 % (1 << 32) for b in range(batch)])
+    Q = Q.astype(np.uint32).reshape(1, batch, cols)
+    got = run_dbmul(D, Q, None, regime)
+    for b in range(batch):
+        assert np.array_equal(got[0, b], Q[0, b, perm]), f"query {b}"
+
+
+@pytest.mark.parametrize("regime", [M1, M2])
+@pytest.mark.parametrize("rows,chunks", [(128, 5), (300, 4), (9700, 3), (19000, 2), (24000, 2)])
+def test_mma_split_units_and_plan_reuse(regime, rows, chunks):
+    """Fewer units than CTAs (every unit dealt out chunk by chunk) up to several rounds plus a
+    leftover round; the same plan is launched repeatedly, so the in-kernel reset of the ticket and
+    arrival counters is exercised too."""
+    import torch
+    ensure_built()
+    cols, batch = 32768 * (chunks - 1) + 4096, 3
+    D = inputs.db_rows(400 + rows, rows, cols, 8)
+    d_db = torch.from_numpy(D).cuda()
+    for moduli in (None, PRIMES):
+        Q = inputs.query(400 + rows, cols, batch, moduli)
+        want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+        d_q = torch.from_numpy(Q.view(np.int32)).cuda()
+        with vipir.Plan(rows, cols, batch, 8, moduli, regime) as plan:
+            assert plan.info["n_chunks"] == chunks
+            for it in range(3):
+                d_a = torch.full((Q.shape[0], batch, rows), -1 - it, dtype=torch.int32, device="cuda")
+                plan(d_db, d_q, d_a)
+                torch.cuda.synchronize()
+                assert_same(d_a.cpu().numpy().view(np.uint32), want)
+
+
 # ---- K chunking: int32 accumulators at their limit (DESIGN.md R7) ------------------------------
 
 @pytest.mark.parametrize("regime", [M1, M2])
