@@ -178,11 +178,12 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     ptx::tc_fence_before();
     if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tmem_base = *tmem_ptr;
+    // same in every lane: say so (shfl from lane 0), so the single-issuer loops run on the uniform datapath
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
 
     if (warp == 0) {
-        // ===== TMA producer =====
-        if (lane == 0) {
+        // ===== TMA producer: the whole warp runs the (warp-uniform) loop, one elected lane issues =====
+        {
             uint32_t sa = 0, pa = 0, sb = 0, pb = 0;
             // H is streamed once when there is a single N tile; sibling N tiles re-read it from L2
             const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
@@ -192,7 +193,9 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 const int32_t row0 = (int32_t)((mt * CG + rank) * MG_BM);
                 for (uint32_t a = 0; a < p.atoms; ++a) {
                     ptx::mbar_wait(&emptyB[sb], pb ^ 1);
+                    __syncwarp();
                     uint8_t* dB = sB_ring + (size_t)sb * p.b_stage_bytes;
+                    if (ptx::elect_one()) {
                     if constexpr (CG == 1) {
                         ptx::mbar_arrive_expect_tx(&fullB[sb], p.b_stage_bytes);
                         ptx::tma_load_4d(dB, &tmB, &fullB[sb], (int32_t)(a * MG_BK), (int32_t)(nt * p.ct), 0,
@@ -204,12 +207,16 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                                               (int32_t)(nt * p.ct), (int32_t)(2 * rank), (int32_t)prob,
                                               ptx::kEvictNormal);
                     }
+                    }
+                    __syncwarp();
                     if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
 #pragma unroll 1
                     for (uint32_t i = 0; i < 4; ++i) {
                         ptx::mbar_wait(&emptyA[sa], pa ^ 1);
+                        __syncwarp();
                         uint8_t* dA = sA_ring + (size_t)sa * MG_A_BYTES;
                         const int32_t kb = (int32_t)((a * 4 + i) * MG_BK);
+                        if (ptx::elect_one()) {
                         if constexpr (CG == 1) {
                             ptx::mbar_arrive_expect_tx(&fullA[sa], MG_A_BYTES);
                             ptx::tma_load_3d(dA, &tmA, &fullA[sa], kb, row0, (int32_t)prob, hintA);
@@ -218,6 +225,8 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                             ptx::tma_load_3d_pair(dA, &tmA, ptx::mapa(ptx::smem_u32(&fullA[sa]), 0), kb, row0,
                                                   (int32_t)prob, hintA);
                         }
+                        }
+                        __syncwarp();
                         if (++sa == p.a_stages) { sa = 0; pa ^= 1; }
                     }
                 }
@@ -225,7 +234,8 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     } else if (warp == 1) {
         // ===== MMA issuer (leader CTA of the pair only) =====
-        if (rank == 0 && lane == 0) {
+        // whole warp in the (warp-uniform) loop; one elected lane -- always the same -- issues and commits
+        if (rank == 0) {
             uint32_t sa = 0, pa = 0, sb = 0, pb = 0, acc_it = 0;
             const uint64_t dZ = make_smem_desc_zero(ptx::smem_u32(sZero));
             for (uint32_t u = unit0; u < n_units; u += unit_stride) {
@@ -246,6 +256,8 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                         for (uint32_t i = 0; i < 4; ++i) {
                             ptx::mbar_wait(&fullA[sa], pa);
                             ptx::tc_fence_after();
+                            __syncwarp();
+                            if (ptx::elect_one()) {
                             const uint64_t dA = make_smem_desc(ptx::smem_u32(sA_ring + (size_t)sa * MG_A_BYTES));
                             const bool first = (a == a_begin && i == 0);
                             // blocks 3..6 start at zero (0 * anything), then H_0*C overwrites blocks 0..3
@@ -258,14 +270,20 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                             }
                             if constexpr (CG == 2) ptx::tc_commit_pair(&emptyA[sa], 3);
                             else ptx::tc_commit(&emptyA[sa]);
+                            if (i == 3) {
+                                if constexpr (CG == 2) ptx::tc_commit_pair(&emptyB[sb], 3);
+                                else ptx::tc_commit(&emptyB[sb]);
+                                if (a + 1 == a_end) {
+                                    if constexpr (CG == 2) ptx::tc_commit_pair(&tmem_full[as], 3);
+                                    else ptx::tc_commit(&tmem_full[as]);
+                                }
+                            }
+                            }
+                            __syncwarp();
                             if (++sa == p.a_stages) { sa = 0; pa ^= 1; }
                         }
-                        if constexpr (CG == 2) ptx::tc_commit_pair(&emptyB[sb], 3);
-                        else ptx::tc_commit(&emptyB[sb]);
                         if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
                     }
-                    if constexpr (CG == 2) ptx::tc_commit_pair(&tmem_full[as], 3);
-                    else ptx::tc_commit(&tmem_full[as]);
                 }
             }
         }
