@@ -14,3 +14,4 @@ from .vipir_oracle import (  # noqa: F401
     lib_path,
 )
 from .modgemm import modgemm, modgemm_bruteforce, modgemm_lazy  # noqa: F401  (NEXT-4)
+from .ntt import ntt_lift, smallest_psi, LAYOUT_G, LAYOUT_H  # noqa: F401  (lift + NTT producing G and H)

@@ -18,7 +18,8 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "vipir_oracle.c"
-_SRCS = [_SRC, _HERE / "vipir_modgemm_oracle.c"]  # NEXT-4: parallel modular GEMMs (own file, same library)
+_SRCS = [_SRC, _HERE / "vipir_modgemm_oracle.c",  # NEXT-4: parallel modular GEMMs (own file, same library)
+         _HERE / "vipir_ntt_oracle.c"]             # lift + forward NTT producing G and H (own file, same library)
 _LIB = _HERE / "libvipir_oracle.so"
 _lib = None
 
@@ -58,6 +59,8 @@ def _load():
         lib.vipir_oracle_modgemm.argtypes = [u32, u64, u64, u64, u64, u64, vp, vp, vp, vp, vp, i32]
         lib.vipir_oracle_modgemm_lazy.restype = ctypes.c_int
         lib.vipir_oracle_modgemm_lazy.argtypes = [u32, u64, u64, u64, u64, u64, vp, vp, vp, vp, vp, u32]
+        lib.vipir_oracle_ntt_lift.restype = ctypes.c_int
+        lib.vipir_oracle_ntt_lift.argtypes = [u32, u32, u32, u32, vp, vp, vp, u32, i32, i32, vp, vp, i32]
         _lib = lib
     return _lib
 
