@@ -255,6 +255,62 @@ int vipir_modgemm_info(const vipir_modgemm_plan *plan, vipir_modgemm_info_t *out
 /* Free the plan and its workspaces.  NULL is a no-op. */
 void vipir_modgemm_destroy(vipir_modgemm_plan *plan);
 
+/* ===========================================================================================
+ * Lift + forward NTT: the scan's scalar-HE words (and, offline, the hint) -> the ring-packing
+ * operands G and H of vipir_modgemm
+ *
+ * PAPER.md:214 (section 3.5.2): "the D1 x n and D1 x B SimplePIR outputs are first transformed into
+ * polynomials by treating each length-N vector along the D1 dimension as a polynomial in R_q ...
+ * to which NTTs are applied independently.  Let H and G denote these two polynomial matrices after
+ * the NTTs."  PAPER.md:667 (Appendix C.1): the server "lifts the coefficients of iota(A_i) and
+ * iota(b) from Z_p to Z_q and transforms them into the NTT domain"; eq. (3) scales
+ * the b part by Delta.  PAPER.md:269-271 (section 4.3): single-kernel NTT for N = 2^12, fused with
+ * the RNS decomposition; layout transposition to the GEMM-friendly layout (fused
+ * into this kernel's store).
+ *
+ * Definition (bit-exact).  d_X [n_a][M][N] uint32: word j of polynomial (a, m); i.e. the layout of
+ * vipir_dbmul's answer [batch = n_a][rows = M*N] after vipir_plan_set_modswitch(plan, p_bits): every
+ * word < p = 2^p_bits.  For RNS prime t (modulus q_t > p, primitive 2N-th root of unity psi_t, scale_t):
+ *     x_j  = scale_t * lift_t(X[a][m][j])  mod q_t
+ *     Y[c] = sum_{j<N} x_j * psi_t^((2c+1) j)  mod q_t,   c < N       (natural order: the polynomial
+ *            evaluated at the c-th odd power of psi_t, the roots of X^N + 1)
+ * lift(x) = x (centered == 0), or x - p taken mod q_t for x >= p/2 (centered == 1).
+ * Output, canonical in [0, q_t):
+ *     VIPIR_NTT_LAYOUT_G:  d_O[t][c][a][m]   = vipir_modgemm's d_G [T][NC = N][gcols = n_a][M]
+ *     VIPIR_NTT_LAYOUT_H:  d_O[t][c][m][a]   = vipir_modgemm's d_H [T][NC = N][M][K = n_a]
+ * Words >= p are a caller error: their excess bits are ignored and a flag is raised that
+ * vipir_ntt_bad_input reads (and clears).
+ * Ownership: the caller owns d_X and d_O (DEVICE pointers, 4-byte aligned, not overlapping); the plan
+ * owns its twiddle tables.  vipir_ntt_lift only enqueues on `cuda_stream`.
+ * =========================================================================================== */
+typedef struct vipir_ntt_plan vipir_ntt_plan;
+#define VIPIR_NTT_LAYOUT_G 0u
+#define VIPIR_NTT_LAYOUT_H 1u
+
+/*
+ * Build a plan (host; computes the twiddle tables psi_t^bitrev(i) and their Shoup companions and
+ * copies them to the current device).
+ *   log2n   log2 N: 4, 8 or 12 (the paper's N = 2^12)
+ *   moduli, psi, scale   HOST pointers to T values: 2^p_bits < q_t < 2^30, psi_t^N = -1 mod q_t,
+ *           scale_t any u32 (reduced mod q_t; 1 for H, Delta mod q_t for G)
+ *   p_bits  1..29 (the paper's p = 2^18)
+ * Errors: INVALID_ARG (null, T == 0 or > VIPIR_MAX_MODULI, modulus out of range, psi not a primitive
+ * 2N-th root of unity, p_bits out of range, centered > 1), UNSUPPORTED (log2n), ARCH, ALLOC, CUDA.
+ */
+int vipir_ntt_plan_create(vipir_ntt_plan **out, uint32_t T, uint32_t log2n, const uint32_t *moduli,
+                          const uint32_t *psi, const uint32_t *scale, uint32_t p_bits, uint32_t centered);
+
+/* Enqueue the transform of n_a * M polynomials.  Errors: INVALID_ARG (null / misaligned pointer, zero
+ * size, out_layout > 1), UNSUPPORTED (n_a * M >= 2^31), CUDA. */
+int vipir_ntt_lift(vipir_ntt_plan *plan, const uint32_t *d_X, uint32_t n_a, uint32_t M, uint32_t out_layout,
+                   uint32_t *d_O, void *cuda_stream);
+
+/* *seen = 1 if any launch since the last call read a word >= 2^p_bits (synchronises the device). */
+int vipir_ntt_bad_input(vipir_ntt_plan *plan, uint32_t *seen);
+
+/* Free the plan and its tables.  NULL is a no-op. */
+void vipir_ntt_destroy(vipir_ntt_plan *plan);
+
 #ifdef __cplusplus
 }
 #endif

@@ -112,7 +112,10 @@ def encrypt(m_poly, s_poly, q: int, delta: int, rng: np.random.Generator, err_bo
     """(a, b) with a*s + b = Delta*m + e mod q; e uniform in [-err_bound, err_bound] (a small
     error stands in for the sigma = 3.2 Gaussian: only |e| < Delta/2 matters)."""
     N = len(s_poly)
-    a = [int(x) for x in rng.integers(0, q, size=N)]
+    if q < (1 << 62):
+        a = [int(x) for x in rng.integers(0, q, size=N)]
+    else:  # an RNS modulus q = q_0 q_1 q_2 ~ 2^87 (PAPER.md:95): 128 random bits reduced mod q
+        a = [int.from_bytes(rng.bytes(16), "little") % q for _ in range(N)]
     e = [int(x) for x in rng.integers(-err_bound, err_bound + 1, size=N)]
     a_s = negacyclic_mul(a, [x % q for x in s_poly], q)
     b = [(delta * int(m_poly[j]) + e[j] - a_s[j]) % q for j in range(N)]

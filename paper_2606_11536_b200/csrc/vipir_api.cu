@@ -534,3 +534,4 @@ void vipir_destroy(vipir_plan* p) {
 }  // extern "C"
 
 #include "modgemm_host.cuh"  // vipir_modgemm_* (parallel INT32 modular GEMMs, NEXT-4)
+#include "ntt_host.cuh"      // vipir_ntt_* (lift + forward NTT producing G and H)

@@ -28,6 +28,7 @@ SYMBOLS = (
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
     "vipir_modgemm_plan_create", "vipir_modgemm_set_h", "vipir_modgemm", "vipir_modgemm_split_c",
     "vipir_modgemm_products", "vipir_modgemm_info", "vipir_modgemm_destroy",
+    "vipir_ntt_plan_create", "vipir_ntt_lift", "vipir_ntt_bad_input", "vipir_ntt_destroy",
 )
 
 
@@ -124,6 +125,15 @@ def load() -> ctypes.CDLL:
         lib.vipir_modgemm_info.argtypes = [vp, ctypes.POINTER(ModGemmInfo)]
         lib.vipir_modgemm_destroy.restype = None
         lib.vipir_modgemm_destroy.argtypes = [vp]
+        u32p = ctypes.POINTER(ctypes.c_uint32)
+        lib.vipir_ntt_plan_create.restype = i
+        lib.vipir_ntt_plan_create.argtypes = [pp, u32, u32, u32p, u32p, u32p, u32, u32]
+        lib.vipir_ntt_lift.restype = i
+        lib.vipir_ntt_lift.argtypes = [vp, vp, u32, u32, u32, vp, vp]
+        lib.vipir_ntt_bad_input.restype = i
+        lib.vipir_ntt_bad_input.argtypes = [vp, u32p]
+        lib.vipir_ntt_destroy.restype = None
+        lib.vipir_ntt_destroy.argtypes = [vp]
         lib.vipir_status_str.restype = ctypes.c_char_p
         lib.vipir_status_str.argtypes = [i]
         lib.vipir_last_cuda_error.restype = ctypes.c_char_p
@@ -305,6 +315,68 @@ class ModGemmPlan:
     def close(self):
         if self.handle is not None:
             modgemm_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ---- lift + forward NTT producing the ring-packing operands G and H (include/vipir.h) ------------
+
+NTT_LAYOUT_G, NTT_LAYOUT_H = 0, 1
+
+
+def ntt_plan_create(log2n: int, moduli, psi, scale, p_bits: int, centered: bool = False):
+    """vipir_ntt_plan_create; returns the opaque plan handle."""
+    T = len(moduli)
+    if len(psi) != T or len(scale) != T:
+        raise ValueError("one psi and one scale per modulus")
+    arr = lambda xs: (ctypes.c_uint32 * max(T, 1))(*[int(x) for x in xs])  # noqa: E731
+    handle = ctypes.c_void_p()
+    _check(load().vipir_ntt_plan_create(ctypes.byref(handle), T, log2n, arr(moduli), arr(psi), arr(scale), p_bits,
+                                        1 if centered else 0), "vipir_ntt_plan_create")
+    return handle
+
+
+def ntt_lift(plan, d_X, n_a: int, M: int, out_layout: int, d_O, stream=None):
+    """vipir_ntt_lift: d_X [n_a][M][N] u32 -> d_O [T][N][n_a][M] (LAYOUT_G) or [T][N][M][n_a] (LAYOUT_H)."""
+    _check(load().vipir_ntt_lift(plan, _ptr(d_X), n_a, M, out_layout, _ptr(d_O), _stream_ptr(stream)), "vipir_ntt_lift")
+
+
+def ntt_bad_input(plan) -> bool:
+    seen = ctypes.c_uint32(0)
+    _check(load().vipir_ntt_bad_input(plan, ctypes.byref(seen)), "vipir_ntt_bad_input")
+    return bool(seen.value)
+
+
+def ntt_destroy(plan):
+    load().vipir_ntt_destroy(plan)
+
+
+class NttPlan:
+    """Context-manager convenience around ntt_plan_create / ntt_destroy."""
+
+    def __init__(self, log2n, moduli, psi, scale, p_bits, centered=False):
+        self.handle = ntt_plan_create(log2n, moduli, psi, scale, p_bits, centered)
+
+    def __call__(self, d_X, n_a, M, out_layout, d_O, stream=None):
+        ntt_lift(self.handle, d_X, n_a, M, out_layout, d_O, stream)
+
+    def bad_input(self) -> bool:
+        return ntt_bad_input(self.handle)
+
+    def close(self):
+        if self.handle is not None:
+            ntt_destroy(self.handle)
             self.handle = None
 
     def __enter__(self):
