@@ -107,3 +107,34 @@ def test_product_never_imports_the_oracle():
     for f in (ROOT / "oracle").rglob("*.py"):
         assert not re.search(r"^\s*(from|import)\s+paper_2606_11536_b200\b", f.read_text(), re.M), f
     assert "#include \"" not in (ROOT / "oracle" / "vipir_oracle.c").read_text()  # system headers only
+
+
+# ---- vipir_ntt_*: argument checks that need no device ------------------------------------------
+
+def _ntt_status(lib, T, log2n, moduli, psi, scale, p_bits, centered=0):
+    h = ctypes.c_void_p()
+    arr = lambda xs: (ctypes.c_uint32 * max(1, len(xs)))(*xs)  # noqa: E731
+    st = lib.vipir_ntt_plan_create(ctypes.byref(h), T, log2n, arr(moduli), arr(psi), arr(scale), p_bits, centered)
+    if st == vipir.OK:
+        lib.vipir_ntt_destroy(h)
+    return st
+
+
+def test_ntt_plan_argument_checks(lib):
+    q, psi16 = 97, 19                     # 19^16 = -1 mod 97: a primitive 32nd root of unity
+    assert pow(psi16, 16, q) == q - 1
+    assert _ntt_status(lib, 0, 4, [q], [psi16], [1], 6) == vipir.ERR_INVALID_ARG            # T == 0
+    assert _ntt_status(lib, 5, 4, [q] * 5, [psi16] * 5, [1] * 5, 6) == vipir.ERR_INVALID_ARG  # T > 4
+    assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 0) == vipir.ERR_INVALID_ARG            # p_bits
+    assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 30) == vipir.ERR_INVALID_ARG
+    assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 7) == vipir.ERR_INVALID_ARG            # p = 128 > q
+    assert _ntt_status(lib, 1, 4, [q], [psi16 * psi16 % q], [1], 6) == vipir.ERR_INVALID_ARG  # order 16, not 32
+    assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 6, centered=2) == vipir.ERR_INVALID_ARG
+    assert _ntt_status(lib, 1, 5, [q], [psi16], [1], 6) == vipir.ERR_UNSUPPORTED            # log2 N not 4/8/12
+    assert lib.vipir_ntt_plan_create(None, 1, 4, None, None, None, 6, 0) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_ntt_lift(None, None, 1, 1, 0, None, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_ntt_bad_input(None, None) == vipir.ERR_INVALID_ARG
+    lib.vipir_ntt_destroy(None)
+    import torch
+    if not torch.cuda.is_available():     # a valid request must fail loudly without a B200, never succeed
+        assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 6) in (vipir.ERR_CUDA, vipir.ERR_ARCH)
