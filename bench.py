@@ -273,6 +273,37 @@ def run_modgemm(B, steps, warmup, peaks):
     }
 
 
+def run_ntt(n_a, layout_name, steps, warmup):
+    """Lift + forward NTT (N = 2^12, the 3 RNS primes) of n_a x 256 polynomials into G or H."""
+    import torch
+    from paper_2606_11536_b200 import vipir
+    from paper_2606_11536_b200.inputs import device
+    N, M, p_bits = 4096, MODGEMM_SHAPE[2], 18
+    psi = [next(x for x in range(2, q) if pow(x, N, q) == q - 1) for q in MODGEMM_PRIMES]
+    q_all = MODGEMM_PRIMES[0] * MODGEMM_PRIMES[1] * MODGEMM_PRIMES[2]
+    scale = [(q_all >> p_bits) % q for q in MODGEMM_PRIMES] if layout_name == "G" else [1, 1, 1]
+    layout = vipir.NTT_LAYOUT_G if layout_name == "G" else vipir.NTT_LAYOUT_H
+    d_X = device.query(SEED, M * N, n_a)[0].view(torch.int32)
+    d_X = (d_X >> (32 - p_bits)) & ((1 << p_bits) - 1)                  # words < 2^18, as after the fused switch
+    T = len(MODGEMM_PRIMES)
+    d_O = torch.empty((T, N, n_a, M) if layout_name == "G" else (T, N, M, n_a), dtype=torch.int32, device="cuda")
+    stream = torch.cuda.current_stream()
+    with vipir.NttPlan(12, MODGEMM_PRIMES, psi, scale, p_bits) as plan:
+        ms = time_events(lambda: plan(d_X, n_a, M, layout, d_O), steps, warmup, stream) / steps
+        bad = plan.bad_input()
+    polys = float(n_a) * M * T
+    # plain-ALU bound (DESIGN.md section 13): a Harvey butterfly needs 4 alu-pipe ops (and 3 fma-pipe
+    # multiplies); each pipe issues 64 lanes per clock per SM (B300_MICROARCH.md "Pipe rates": rt_SMSP = 2)
+    lane_ops = polys * 24576 * 4
+    peak = 148 * 64 * 1.965e9
+    alg_bytes = 4.0 * n_a * M * N * (1 + T)
+    return {"workload": f"{n_a} x {M} polynomials, N = 4096, {T} primes -> {layout_name}", "ms": ms, "bad_input": bad,
+            "transforms_per_s": polys / ms * 1e3, "GBps_in_plus_out": alg_bytes / ms / 1e6,
+            "roofline": {"bound": "alu", "kernel": "ntt_lift_kernel<12>", "achieved": lane_ops / ms / 1e9,
+                         "peak": peak / 1e12, "unit": "T alu-pipe lane-op/s (INT32)", "frac": lane_ops / ms * 1e3 / peak,
+                         "traffic": profiled_traffic("ntt_lift_kernel_G_B32") if (n_a, layout_name) == (32, "G") else None}}
+
+
 def cpu_baseline(sample_rows: int, device_db, cols: int):
     """The oracle, as it stands, on the host cores, on the first `sample_rows` rows of the
     headline workload (same bytes: copied back from the device-generated DB)."""
@@ -365,6 +396,8 @@ def run_cuda(args):
             del buf
             torch.cuda.empty_cache()
             extra["modgemm"] = {f"B{B}": run_modgemm(B, max(10, args.steps // 5), 3, peaks) for B in (1, 8, 32)}
+            extra["ntt"] = {"G_B1": run_ntt(1, "G", 50, 5), "G_B32": run_ntt(32, "G", 50, 5),
+                            "H_n1280_offline": run_ntt(1280, "H", 3, 1)}
 
     if rank == 0:
         b = extra.get(BATCHED)
@@ -404,6 +437,8 @@ def run_cuda(args):
             }
         if "modgemm" in extra:
             line["modgemm"] = extra.pop("modgemm")
+        if "ntt" in extra:
+            line["ntt"] = extra.pop("ntt")
         if args.all or args.paper:
             line["configs"] = {n: {k: v for k, v in r.items() if k not in ("alg_bytes", "int8_ops")} for n, r in extra.items()}
             line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in ("alg_bytes", "int8_ops")}
@@ -457,7 +492,7 @@ def main():
     ap.add_argument("--all", action="store_true", help="also time every other BASELINE.json config")
     ap.add_argument("--paper", action="store_true", help="also time the paper's Table-2 shapes and NEXT-2 shapes (64 GiB DB)")
     ap.add_argument("--modgemm", action="store_true",
-                    help="also time the parallel modular GEMMs H*C+(0|G) at the paper's 64 GiB shape (NEXT-4)")
+                    help="also time the ring-packing stage at the paper's 64 GiB shape: lift + NTT (G, H) and H*C+(0|G)")
     ap.add_argument("--cpu-sample-rows", type=int, default=32768)
     ap.add_argument("--ref-sample-rows", type=int, default=4096)
     args = ap.parse_args()
