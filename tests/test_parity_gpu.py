@@ -198,6 +198,36 @@ def test_mma_split_units_and_plan_reuse(regime, rows, chunks):
                 assert_same(d_a.cpu().numpy().view(np.uint32), want)
 
 
+def test_cuda_graph_replay_of_split_units():
+    """vipir_dbmul only enqueues (include/vipir.h): it can be captured into a CUDA graph, and the
+    in-kernel reset of the ticket / arrival counters makes every replay start from a clean state."""
+    import torch
+    ensure_built()
+    rows, cols, batch = 9700, 32768 * 2 + 4096, 3           # units dealt out chunk by chunk (see above)
+    D = inputs.db_rows(431, rows, cols, 8)
+    d_db = torch.from_numpy(D).cuda()
+    for moduli in (None, PRIMES):
+        Q = inputs.query(431, cols, batch, moduli)
+        want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+        d_q = torch.from_numpy(Q.view(np.int32)).cuda()
+        d_a = torch.zeros((Q.shape[0], batch, rows), dtype=torch.int32, device="cuda")
+        with vipir.Plan(rows, cols, batch, 8, moduli, M2) as plan:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                plan(d_db, d_q, d_a, stream=side)             # warm-up outside capture
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                plan(d_db, d_q, d_a, stream=side)
+            for it in range(3):
+                d_a.fill_(-1 - it)
+                graph.replay()
+                torch.cuda.synchronize()
+                assert_same(d_a.cpu().numpy().view(np.uint32), want)
+
+
 # ---- K chunking: int32 accumulators at their limit (DESIGN.md R7) ------------------------------
 
 @pytest.mark.parametrize("regime", [M1, M2])
