@@ -42,8 +42,9 @@ int launch_ntt(vipir_ntt_plan* p, const vipir::NttParams& np, cudaStream_t st) {
     }
     const uint64_t groups = (uint64_t)np.n_outer * ((np.n_inner + P - 1) / P);
     // the twiddle tables are loaded once per CTA: a CTA takes several polynomial groups when there are many
-    uint32_t gx = (uint32_t)(groups < (uint64_t)p->num_sms * 4 ? groups : (uint64_t)p->num_sms * 4);
-    if (L == 12 && gx > (uint32_t)p->num_sms * 2) gx = (uint32_t)p->num_sms * 2;
+    // (N = 4096: one CTA per SM is resident, so one CTA per SM and prime is launched)
+    const uint64_t cap = (uint64_t)p->num_sms * (L == 12 ? 1 : 4);
+    const uint32_t gx = (uint32_t)(groups < cap ? groups : cap);
     kern<<<dim3(gx, p->T), vipir::NTT_THREADS, smem, st>>>(np);
     CK(cudaGetLastError());
     return VIPIR_OK;

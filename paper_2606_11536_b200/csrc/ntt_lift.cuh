@@ -80,6 +80,18 @@ __device__ __forceinline__ void radix16_pass(uint32_t (&r)[16], uint32_t rho, ui
     }
 }
 
+// barrier among the TP threads of one polynomial.  For N = 4096 (TP = 256: whole warps) it is a named
+// barrier of its own, so the Q polynomials in flight drift out of phase and one's global loads and
+// barrier waits overlap the other's butterflies; smaller N (sub-warp groups) use the CTA barrier.
+template <uint32_t TP>
+__device__ __forceinline__ void ntt_group_sync(uint32_t group) {
+    if constexpr (TP % 32 == 0 && TP < NTT_THREADS) {
+        asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(TP) : "memory");
+    } else {
+        __syncthreads();
+    }
+}
+
 __device__ __forceinline__ uint32_t ntt_pad(uint32_t i) { return i + (i >> 4); }   // work buffer
 __device__ __forceinline__ uint32_t ntt_pad_out(uint32_t c) { return c + (c >> 5); }  // natural-order staging
 
@@ -115,6 +127,23 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
     for (uint32_t grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
         const uint32_t outer = grp / groups_per_outer;
         const uint32_t inner0 = (grp % groups_per_outer) * P;
+        // this thread's 16 input words of round rd, prefetched into the round's (still unused) work slot
+        // with cp.async one round ahead: the global-load latency overlaps the previous round's butterflies
+        auto prefetch = [&](uint32_t rd) {
+            const uint32_t slot = rd * Q + slot0;
+            const uint32_t inner = inner0 + slot;
+            if (rd < R && inner < p.n_inner) {
+                const uint32_t* src =
+                    p.X + ((size_t)outer * p.in_stride_outer + (size_t)inner * p.in_stride_inner) * N + tid;
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(buf + slot * STR + tid);
+#pragma unroll
+                for (int k = 0; k < 16; ++k)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + k * TP * 4), "l"(src + k * TP)
+                                 : "memory");
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        prefetch(0);
 #pragma unroll 1
         for (uint32_t rd = 0; rd < R; ++rd) {
             const uint32_t slot = rd * Q + slot0;
@@ -122,48 +151,61 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
             const bool live = inner < p.n_inner;
             uint32_t* work = buf + slot * STR;
             uint32_t r[16];
-            // ---- pass 0: global -> lift -> scale -> stages 0..3 ----
+            prefetch(rd + 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            // ---- pass 0: lift -> scale -> stages 0..3 ----
             {
-                const uint32_t* src =
-                    p.X + ((size_t)outer * p.in_stride_outer + (size_t)inner * p.in_stride_inner) * N + tid;
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {
-                    uint32_t v = live ? __ldg(src + k * TP) : 0u;
+                    uint32_t v = live ? work[k * TP + tid] : 0u;   // this thread's own cp.async data
                     bad |= v & ~pmask;
                     v &= pmask;
                     if (p.centered && v >= half_p) v = v - (pmask + 1u) + q;  // x - p, taken mod q
                     r[k] = shoup_mul(v, p.scale[t], p.scale_shoup[t], q);      // [0, 2q)
                 }
+                ntt_group_sync<TP>(slot0);  // the slot is reused for the exchange below
                 radix16_pass(r, 0, 0, tw, tws, q);
             }
 #pragma unroll
             for (uint32_t rho = 1; rho < PASSES; ++rho) {
-                // elements of pass rho-1: idx = hi' * 2^(L-4(rho-1)) + k * 2^(L-4rho) + lo'
+                // elements of pass rho-1: idx = hi' * 2^(L-4(rho-1)) + k * 2^(L-4rho) + lo'; the padded index
+                // i + i/16 is linear in k whenever k's stride is a multiple of 16
                 {
-                    const uint32_t lo_bits = L - 4 * rho;  // bits of lo' = bits below k in the previous pass
+                    const uint32_t lo_bits = L - 4 * rho;  // >= 4: bits of lo' = bits below k in the previous pass
                     const uint32_t lo = tid & ((1u << lo_bits) - 1u), hi = tid >> lo_bits;
+                    uint32_t* w0 = work + ntt_pad((hi << (lo_bits + 4)) + lo);
 #pragma unroll
-                    for (int k = 0; k < 16; ++k)
-                        work[ntt_pad((hi << (lo_bits + 4)) + ((uint32_t)k << lo_bits) + lo)] = r[k];
+                    for (int k = 0; k < 16; ++k) w0[k * ((1u << lo_bits) + (1u << (lo_bits - 4)))] = r[k];
                 }
-                __syncthreads();
+                ntt_group_sync<TP>(slot0);
                 const uint32_t lo_bits = L - 4 * rho - 4;
                 const uint32_t lo = tid & ((1u << lo_bits) - 1u), hi = tid >> lo_bits;
+                if (lo_bits >= 4) {
+                    const uint32_t* r0 = work + ntt_pad((hi << (lo_bits + 4)) + lo);
 #pragma unroll
-                for (int k = 0; k < 16; ++k) r[k] = work[ntt_pad((hi << (lo_bits + 4)) + ((uint32_t)k << lo_bits) + lo)];
-                __syncthreads();
+                    for (int k = 0; k < 16; ++k) r[k] = r0[k * ((1u << lo_bits) + ((1u << lo_bits) >> 4))];
+                } else {  // lo_bits == 0: idx = 16 hi + k, padded 17 hi + k
+                    const uint32_t* r0 = work + hi * 17;
+#pragma unroll
+                    for (int k = 0; k < 16; ++k) r[k] = r0[k];
+                }
+                ntt_group_sync<TP>(slot0);
                 radix16_pass(r, rho, hi, tw, tws, q);
             }
-            // ---- normalise to [0, q) and stage in natural order: position pos holds Y[bitrev(pos)] ----
+            // ---- normalise to [0, q) and stage in natural order: position pos = 16 hi + k holds
+            // Y[bitrev(pos)], bitrev(pos) = bitrev4(k) * N/16 + bitrev(hi) ----
             {
-                const uint32_t hi = tid;  // last pass: lo has no bits
+                const uint32_t c0 = (L > 4) ? (__brev(tid) >> (32 - (L > 4 ? L - 4 : 1))) : 0u;
+                uint32_t* s0 = work + ntt_pad_out(c0);
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {
                     uint32_t v = r[k];
                     v = min(v, v - 2 * q);
                     v = min(v, v - q);
-                    const uint32_t c = __brev(hi * 16 + k) >> (32 - L);
-                    work[ntt_pad_out(c)] = v;
+                    constexpr uint32_t kStep = N / 16 + N / 512;  // N/16 padded (a multiple of 32 for N = 4096)
+                    const uint32_t kr = ((k & 1) << 3) | ((k & 2) << 1) | ((k & 4) >> 1) | ((k & 8) >> 3);
+                    if constexpr (L == 12) s0[kr * kStep] = v;
+                    else work[ntt_pad_out(c0 + kr * (N / 16))] = v;
                 }
             }
         }
@@ -173,9 +215,22 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
             const uint32_t n_live = min(P, p.n_inner - inner0);
             uint32_t* dst = p.O + ((size_t)t * N * p.n_outer + outer) * p.n_inner + inner0;
             const size_t c_stride = (size_t)p.n_outer * p.n_inner;
-            for (uint32_t i = threadIdx.x; i < N * P; i += NTT_THREADS) {
-                const uint32_t s = i % P, c = i / P;
-                if (s < n_live) dst[(size_t)c * c_stride + s] = buf[s * STR + ntt_pad_out(c)];
+            const bool vec = (P % 4 == 0) && n_live == P && (p.n_inner % 4 == 0) &&
+                             ((reinterpret_cast<uintptr_t>(p.O) & 15) == 0);
+            if (vec) {
+                // one thread = one c and four neighbouring polynomials: a 16-byte store
+                constexpr uint32_t QUADS = P / 4;
+                for (uint32_t i = threadIdx.x; i < N * QUADS; i += NTT_THREADS) {
+                    const uint32_t c = i / QUADS, s4 = (i % QUADS) * 4;
+                    const uint32_t* src = buf + s4 * STR + ntt_pad_out(c);
+                    const uint4 v = make_uint4(src[0], src[STR], src[2 * STR], src[3 * STR]);
+                    *reinterpret_cast<uint4*>(dst + (size_t)c * c_stride + s4) = v;
+                }
+            } else {
+                for (uint32_t i = threadIdx.x; i < N * P; i += NTT_THREADS) {
+                    const uint32_t s = i % P, c = i / P;
+                    if (s < n_live) dst[(size_t)c * c_stride + s] = buf[s * STR + ntt_pad_out(c)];
+                }
             }
         }
         __syncthreads();
