@@ -304,6 +304,51 @@ def run_ntt(n_a, layout_name, steps, warmup):
                          "traffic": profiled_traffic("ntt_lift_kernel_G_B32") if (n_a, layout_name) == (32, "G") else None}}
 
 
+def run_pipeline(B, steps, warmup):
+    """The built chain at the paper's 64 GiB hybrid shape (N x D_r x D0 = 2^12 x 2^8 x 2^16):
+    (1) scan of the 64 GiB DB for B clients with the fused 2^32 -> 2^18 switch, lift + NTT of its output into G,
+    (3) H*C + (0|G) over the 15 GiB hint -- everything of the online server path except the expansion that
+    produces C and the poly-HE folding (7)."""
+    import torch
+    from paper_2606_11536_b200 import vipir
+    from paper_2606_11536_b200.inputs import device, generator
+    T, NC, M, K = MODGEMM_SHAPE
+    N, p_bits = NC, 18
+    rows, cols = N * M, 1 << 16
+    stream = torch.cuda.current_stream()
+    d_db = device.db(SEED, rows, cols, 8)
+    d_q = device.query(SEED, cols, B)
+    d_a = torch.empty((1, B, rows), dtype=torch.int32, device="cuda")
+    d_G = torch.empty((T, N, B, M), dtype=torch.int32, device="cuda")
+    d_O = torch.empty((T, NC, 2 * B, M), dtype=torch.int32, device="cuda")
+    d_C = device.modgemm_operand(SEED, generator.STREAM_MG_C, MODGEMM_PRIMES, NC, 2 * B * K)
+    psi = [next(x for x in range(2, q) if pow(x, N, q) == q - 1) for q in MODGEMM_PRIMES]
+    q_all = MODGEMM_PRIMES[0] * MODGEMM_PRIMES[1] * MODGEMM_PRIMES[2]
+    scale = [(q_all >> p_bits) % q for q in MODGEMM_PRIMES]
+    with vipir.Plan(rows, cols, B, 8, None, modswitch_bits=p_bits) as scan, \
+            vipir.NttPlan(12, MODGEMM_PRIMES, psi, scale, p_bits) as ntt, \
+            vipir.ModGemmPlan(T, NC, M, K, 2 * B, B, MODGEMM_PRIMES) as mg:
+        d_H = device.modgemm_operand(SEED, generator.STREAM_MG_H, MODGEMM_PRIMES, NC, M * K)
+        mg.set_h(d_H)
+        torch.cuda.synchronize()
+        del d_H
+
+        def step():
+            scan(d_db, d_q, d_a)
+            ntt(d_a, B, M, vipir.NTT_LAYOUT_G, d_G)
+            mg(d_C, d_G, d_O)
+        ms = time_events(step, steps, warmup, stream) / steps
+        ms_scan = time_events(lambda: scan(d_db, d_q, d_a), steps, warmup, stream) / steps
+        ms_ntt = time_events(lambda: ntt(d_a, B, M, vipir.NTT_LAYOUT_G, d_G), steps, warmup, stream) / steps
+        ms_mg = time_events(lambda: mg(d_C, d_G, d_O), steps, warmup, stream) / steps
+        bad = ntt.bad_input()
+        regime = scan.info["regime_name"]
+    return {"workload": f"64 GiB u8 DB 2^20 x 2^16, B = {B}; N = 4096, D_r = 256, n = 1280, 3 RNS primes",
+            "ms_per_batch": ms, "queries_per_s": B / ms * 1e3, "ms_scan": ms_scan, "ms_ntt_G": ms_ntt,
+            "ms_modgemm": ms_mg, "scan_regime": regime, "kernels_per_batch": 5, "ntt_bad_input": bad,
+            "resident_GB": (rows * cols + 4.0 * T * NC * M * 1280) / 1e9}
+
+
 def cpu_baseline(sample_rows: int, device_db, cols: int):
     """The oracle, as it stands, on the host cores, on the first `sample_rows` rows of the
     headline workload (same bytes: copied back from the device-generated DB)."""
@@ -398,6 +443,11 @@ def run_cuda(args):
             extra["modgemm"] = {f"B{B}": run_modgemm(B, max(10, args.steps // 5), 3, peaks) for B in (1, 8, 32)}
             extra["ntt"] = {"G_B1": run_ntt(1, "G", 50, 5), "G_B32": run_ntt(32, "G", 50, 5),
                             "H_n1280_offline": run_ntt(1280, "H", 3, 1)}
+        if args.pipeline:
+            if "buf" in locals():
+                del buf
+            torch.cuda.empty_cache()
+            extra["pipeline"] = {f"B{B}": run_pipeline(B, max(10, args.steps // 5), 3) for B in (1, 8, 32)}
 
     if rank == 0:
         b = extra.get(BATCHED)
@@ -439,6 +489,8 @@ def run_cuda(args):
             line["modgemm"] = extra.pop("modgemm")
         if "ntt" in extra:
             line["ntt"] = extra.pop("ntt")
+        if "pipeline" in extra:
+            line["pipeline"] = extra.pop("pipeline")
         if args.all or args.paper:
             line["configs"] = {n: {k: v for k, v in r.items() if k not in ("alg_bytes", "int8_ops")} for n, r in extra.items()}
             line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in ("alg_bytes", "int8_ops")}
@@ -493,6 +545,8 @@ def main():
     ap.add_argument("--paper", action="store_true", help="also time the paper's Table-2 shapes and NEXT-2 shapes (64 GiB DB)")
     ap.add_argument("--modgemm", action="store_true",
                     help="also time the ring-packing stage at the paper's 64 GiB shape: lift + NTT (G, H) and H*C+(0|G)")
+    ap.add_argument("--pipeline", action="store_true",
+                    help="also time the built chain scan -> NTT -> H*C+(0|G) at the paper's 64 GiB hybrid shape")
     ap.add_argument("--cpu-sample-rows", type=int, default=32768)
     ap.add_argument("--ref-sample-rows", type=int, default=4096)
     args = ap.parse_args()
