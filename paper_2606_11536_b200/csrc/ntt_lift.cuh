@@ -65,6 +65,7 @@ __device__ __forceinline__ void harvey_butterfly(uint32_t& x, uint32_t& y, uint3
 
 // four radix-2 stages (one radix-16 step) on r[0..15]; pass rho covers stages 4*rho .. 4*rho+3,
 // `hi` = the element index bits above this group's 4 bits.  tw/tws: the prime's tables (shared memory).
+template <bool TW_SMEM>
 __device__ __forceinline__ void radix16_pass(uint32_t (&r)[16], uint32_t rho, uint32_t hi, const uint32_t* tw,
                                              const uint32_t* tws, uint32_t q) {
 #pragma unroll
@@ -73,7 +74,8 @@ __device__ __forceinline__ void radix16_pass(uint32_t (&r)[16], uint32_t rho, ui
         const uint32_t base = (1u << (4 * rho + sigma)) + (hi << sigma);
 #pragma unroll
         for (int b = 0; b < (1 << sigma); ++b) {
-            const uint32_t w = tw[base + b], ws = tws[base + b];
+            const uint32_t w = TW_SMEM ? tw[base + b] : __ldg(tw + base + b);
+            const uint32_t ws = TW_SMEM ? tws[base + b] : __ldg(tws + base + b);
 #pragma unroll
             for (int k = 0; k < half; ++k) harvey_butterfly(r[b * 2 * half + k], r[b * 2 * half + k + half], w, ws, q);
         }
@@ -83,9 +85,9 @@ __device__ __forceinline__ void radix16_pass(uint32_t (&r)[16], uint32_t rho, ui
 // barrier among the TP threads of one polynomial.  For N = 4096 (TP = 256: whole warps) it is a named
 // barrier of its own, so the Q polynomials in flight drift out of phase and one's global loads and
 // barrier waits overlap the other's butterflies; smaller N (sub-warp groups) use the CTA barrier.
-template <uint32_t TP>
+template <uint32_t TP, uint32_t NT>
 __device__ __forceinline__ void ntt_group_sync(uint32_t group) {
-    if constexpr (TP % 32 == 0 && TP < NTT_THREADS) {
+    if constexpr (TP % 32 == 0 && TP < NT) {
         asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(TP) : "memory");
     } else {
         __syncthreads();
@@ -95,26 +97,34 @@ __device__ __forceinline__ void ntt_group_sync(uint32_t group) {
 __device__ __forceinline__ uint32_t ntt_pad(uint32_t i) { return i + (i >> 4); }   // work buffer
 __device__ __forceinline__ uint32_t ntt_pad_out(uint32_t c) { return c + (c >> 5); }  // natural-order staging
 
-// L = log2 N in {4, 8, 12}.  TP = N/16 threads per polynomial, Q = NTT_THREADS / TP polynomials in
-// flight, R rounds: P = Q*R polynomials (neighbours along `inner`) per CTA iteration.
-template <int L>
-__global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
+// L = log2 N in {4, 8, 12}.  NT threads per CTA, TP = N/16 threads per polynomial, Q = NT / TP
+// polynomials in flight, R rounds: P = Q*R polynomials (neighbours along `inner`) per CTA iteration.
+// TW_SMEM: twiddle tables copied to shared memory (small N), or read through L1 (N = 4096, where the
+// shared memory goes to the work slots so that MINB CTAs fit on an SM and their multiply-dense and
+// shared-memory-dense phases overlap).
+template <int L, int NT, int R_, bool TW_SMEM, int MINB>
+__global__ void __launch_bounds__(NT, MINB) ntt_lift_kernel(NttParams p) {
     constexpr uint32_t N = 1u << L;
     constexpr uint32_t TP = N / 16;
-    constexpr uint32_t Q = NTT_THREADS / TP;
-    constexpr uint32_t R = (L == 12) ? 4 : 1;
+    constexpr uint32_t Q = NT / TP;
+    constexpr uint32_t R = R_;
     constexpr uint32_t P = Q * R;
+    constexpr uint32_t NTT_THREADS = NT;
     constexpr uint32_t PASSES = L / 4;
     constexpr uint32_t STR = N + N / 16 + 4;  // words per polynomial slot: padded, and = 4 mod 32 for N >= 512
     extern __shared__ uint32_t ntt_smem[];
-    uint32_t* tw = ntt_smem;         // [N]
-    uint32_t* tws = tw + N;          // [N]
-    uint32_t* buf = tws + N;         // [P][STR]
-
     const uint32_t t = blockIdx.y;
     const uint32_t q = p.moduli[t];
-    for (uint32_t i = threadIdx.x; i < 2 * N; i += NTT_THREADS) tw[i] = p.twiddles[(size_t)t * 2 * N + i];
-    __syncthreads();
+    const uint32_t* tw = p.twiddles + (size_t)t * 2 * N;   // [N] w, then [N] floor(w * 2^32 / q)
+    uint32_t* buf = ntt_smem;                               // [P][STR]
+    if constexpr (TW_SMEM) {
+        uint32_t* tw_s = ntt_smem;
+        buf = ntt_smem + 2 * N;
+        for (uint32_t i = threadIdx.x; i < 2 * N; i += NTT_THREADS) tw_s[i] = tw[i];
+        tw = tw_s;
+        __syncthreads();
+    }
+    const uint32_t* tws = tw + N;
 
     const uint32_t tid = threadIdx.x % TP;   // thread within its polynomial
     const uint32_t slot0 = threadIdx.x / TP; // polynomial slot within a round
@@ -163,8 +173,8 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
                     if (p.centered && v >= half_p) v = v - (pmask + 1u) + q;  // x - p, taken mod q
                     r[k] = shoup_mul(v, p.scale[t], p.scale_shoup[t], q);      // [0, 2q)
                 }
-                ntt_group_sync<TP>(slot0);  // the slot is reused for the exchange below
-                radix16_pass(r, 0, 0, tw, tws, q);
+                ntt_group_sync<TP, NT>(slot0);  // the slot is reused for the exchange below
+                radix16_pass<TW_SMEM>(r, 0, 0, tw, tws, q);
             }
 #pragma unroll
             for (uint32_t rho = 1; rho < PASSES; ++rho) {
@@ -177,7 +187,7 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
 #pragma unroll
                     for (int k = 0; k < 16; ++k) w0[k * ((1u << lo_bits) + (1u << (lo_bits - 4)))] = r[k];
                 }
-                ntt_group_sync<TP>(slot0);
+                ntt_group_sync<TP, NT>(slot0);
                 const uint32_t lo_bits = L - 4 * rho - 4;
                 const uint32_t lo = tid & ((1u << lo_bits) - 1u), hi = tid >> lo_bits;
                 if (lo_bits >= 4) {
@@ -189,8 +199,8 @@ __global__ void __launch_bounds__(NTT_THREADS, 1) ntt_lift_kernel(NttParams p) {
 #pragma unroll
                     for (int k = 0; k < 16; ++k) r[k] = r0[k];
                 }
-                ntt_group_sync<TP>(slot0);
-                radix16_pass(r, rho, hi, tw, tws, q);
+                ntt_group_sync<TP, NT>(slot0);
+                radix16_pass<TW_SMEM>(r, rho, hi, tw, tws, q);
             }
             // ---- normalise to [0, q) and stage in natural order: position pos = 16 hi + k holds
             // Y[bitrev(pos)], bitrev(pos) = bitrev4(k) * N/16 + bitrev(hi) ----
