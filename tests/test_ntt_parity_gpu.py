@@ -135,3 +135,30 @@ def test_chain_scan_ntt_modgemm_decrypts():
             phases = rlwe.decrypt(parts[0], parts[1], ring_secrets[b_], q, delta, p)   # LWE phases mod 2^18
             got = [((ph + (delta_lwe >> 1)) // delta_lwe) & 0xFF for ph in phases]
             assert got == [int(x) for x in D[m * N:(m + 1) * N, targets[b_]]], (b_, m)
+
+
+@pytest.mark.parametrize("n_a,M,layout", [(32, 256, vipir.NTT_LAYOUT_G), (1280, 8, vipir.NTT_LAYOUT_H)])
+def test_ntt_paper_shape_sampled_polynomials_and_coefficient_sums(n_a, M, layout):
+    """The launch configuration bench.py times (N = 2^12, three primes, Delta scale; G for 32 clients x 256
+    polynomials, H columns = 1280): sampled polynomials recomputed one by one by the oracle, plus an identity
+    that covers every polynomial at any size: sum_c Y[c] = N * scale * lift(x_0) mod q, because
+    sum_c psi^((2c+1) j) = 0 for 0 < j < N (psi^(2j) is a non-trivial N-th root of unity)."""
+    N, log2n, p_bits = 4096, 12, 18
+    psi = [oracle.smallest_psi(N, q) for q in Q29]
+    q_all = Q29[0] * Q29[1] * Q29[2]
+    scale = [(q_all >> p_bits) % q for q in Q29]
+    X = (inputs.query(5, M * N, n_a) >> np.uint32(32 - p_bits))[0]       # [n_a][M*N] words < 2^18
+    got, bad = run_ntt(X, log2n, Q29, psi, scale, p_bits, True, layout)
+    assert not bad
+    polys = got if layout == vipir.NTT_LAYOUT_G else got.transpose(0, 1, 3, 2)      # [T][N][n_a][M]
+    g = np.random.default_rng(8)
+    picks = {(0, 0), (n_a - 1, M - 1), (n_a - 1, 0), (0, M - 1)} | {(int(g.integers(n_a)), int(g.integers(M))) for _ in range(4)}
+    for a, m in sorted(picks):
+        want = oracle.ntt_lift(X[a:a + 1, m * N:(m + 1) * N], N, Q29, psi, scale, p_bits, True, oracle.LAYOUT_G, nthreads=16)
+        assert np.array_equal(polys[:, :, a, m], want[:, :, 0, 0]), (a, m)
+    x0 = X.reshape(n_a, M, N)[:, :, 0].astype(np.int64)
+    lifted = np.where(x0 >= (1 << (p_bits - 1)), x0 - (1 << p_bits), x0)
+    for t, q in enumerate(Q29):
+        sums = polys[t].astype(np.uint64).sum(axis=0) % q                  # [n_a][M]
+        want = np.array([[(N * scale[t] * int(v)) % q for v in row] for row in lifted], dtype=np.uint64)
+        assert np.array_equal(sums, want), t
