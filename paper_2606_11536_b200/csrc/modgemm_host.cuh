@@ -196,7 +196,7 @@ int vipir_modgemm_plan_create(vipir_modgemm_plan** out, uint32_t T, uint64_t NC,
     for (uint32_t t = 0; t < T; ++t) p->moduli[t] = moduli[t];
     // CTA pairs (one 256-row tile, each CTA staging half of the C limb tile) once the C tile is wide
     // enough for its shared-memory traffic to matter; VIPIR_TUNE_MG_CG overrides
-    p->cg = (M > 128 && ncols > 16) ? 2u : 1u;
+    p->cg = (M > 128 && ncols >= 16) ? 2u : 1u;  // measured: pairs win from 16 columns up (8 clients: 2.64 -> 2.55 ms)
     const uint32_t cg_force = tune_env("VIPIR_TUNE_MG_CG", 0);
     if (cg_force == 1 || cg_force == 2) p->cg = cg_force;
     p->hp_bytes = p->P * M * 4ull * p->Kp;
