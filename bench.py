@@ -57,6 +57,8 @@ PAPER_CONFIGS = {
     "P_64GiB_B1": (262144, 262144, 1, 8, False),
     "N2_hint_4GiB_B1280": (65536, 65536, 1280, 8, False),
     "N2_tall_64GiB_B1": (1 << 20, 65536, 1, 8, False),
+    # DoublePIR / double-packing second folding, one client: (8N x D1) INT8 by D1 x (n+1) INT32
+    "N2_fold2_4GiB_B1281": (32768, 131072, 1281, 8, False),
 }
 PAPER_QPS_H100 = {"P_1GiB_B32": 8244, "P_4GiB_B32": 2201, "P_16GiB_B32": 565, "P_64GiB_B32": 144}
 HEADLINE = "C3_16GiB_B1"
