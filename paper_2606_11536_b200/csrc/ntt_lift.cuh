@@ -143,13 +143,22 @@ __global__ void __launch_bounds__(NT, MINB) ntt_lift_kernel(NttParams p) {
             const uint32_t slot = rd * Q + slot0;
             const uint32_t inner = inner0 + slot;
             if (rd < R && inner < p.n_inner) {
-                const uint32_t* src =
-                    p.X + ((size_t)outer * p.in_stride_outer + (size_t)inner * p.in_stride_inner) * N + tid;
-                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(buf + slot * STR + tid);
+                const uint32_t* src = p.X + ((size_t)outer * p.in_stride_outer + (size_t)inner * p.in_stride_inner) * N;
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(buf + slot * STR);
+                if (STR % 4 == 0 && (reinterpret_cast<uintptr_t>(p.X) & 15) == 0) {  // slots 16-byte aligned
+                    // the polynomial copied as it lies (16 bytes per thread and step, coalesced)
 #pragma unroll
-                for (int k = 0; k < 16; ++k)
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + k * TP * 4), "l"(src + k * TP)
-                                 : "memory");
+                    for (int i = 0; i < 4; ++i)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + (i * TP + tid) * 16),
+                                     "l"(src + (i * TP + tid) * 4)
+                                     : "memory");
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 16; ++k)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (k * TP + tid) * 4),
+                                     "l"(src + k * TP + tid)
+                                     : "memory");
+                }
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
         };
@@ -163,11 +172,12 @@ __global__ void __launch_bounds__(NT, MINB) ntt_lift_kernel(NttParams p) {
             uint32_t r[16];
             prefetch(rd + 1);
             asm volatile("cp.async.wait_group 1;" ::: "memory");
+            ntt_group_sync<TP, NT>(slot0);  // the words were copied by other threads of the polynomial
             // ---- pass 0: lift -> scale -> stages 0..3 ----
             {
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {
-                    uint32_t v = live ? work[k * TP + tid] : 0u;   // this thread's own cp.async data
+                    uint32_t v = live ? work[k * TP + tid] : 0u;
                     bad |= v & ~pmask;
                     v &= pmask;
                     if (p.centered && v >= half_p) v = v - (pmask + 1u) + q;  // x - p, taken mod q
@@ -230,6 +240,7 @@ __global__ void __launch_bounds__(NT, MINB) ntt_lift_kernel(NttParams p) {
             if (vec) {
                 // one thread = one c and four neighbouring polynomials: a 16-byte store
                 constexpr uint32_t QUADS = P / 4;
+#pragma unroll 4
                 for (uint32_t i = threadIdx.x; i < N * QUADS; i += NTT_THREADS) {
                     const uint32_t c = i / QUADS, s4 = (i % QUADS) * 4;
                     const uint32_t* src = buf + s4 * STR + ntt_pad_out(c);
