@@ -422,6 +422,9 @@ def run_cuda(args):
         dist.all_gather(gathered, t)
         times = [float(g[0]) for g in gathered]
         e2e_times = [float(g[1]) for g in gathered]
+    # read-only ceiling of this part, measured live on the same buffer (plain 128-bit loads, data discarded)
+    ro_ms = time_events(lambda: device.read_only(buf[:nbytes]), 10, 3, torch.cuda.current_stream()) / 10
+    read_only_gbs = nbytes / ro_ms / 1e6
     value, ms_per_step = aggregate(times, nbytes / 1e9, args.steps)
     e2e_value, _ = aggregate(e2e_times, nbytes / 1e9, args.steps)
 
@@ -470,6 +473,8 @@ def run_cuda(args):
                          if peaks["source"] == "measured" else "fallback 6650 GB/s (B200_PROFILING.md)",
                          "unit": "GB/s", "frac": head["frac_hbm_measured"],
                          "frac_of_nominal_8TBps": head["scan_kernel_GBps"] / 8000.0,
+                         "read_only_ceiling_GBps": read_only_gbs,
+                         "frac_of_read_only_ceiling": head["scan_kernel_GBps"] / read_only_gbs,
                          "ms_per_launch": head["ms_scan_kernel"], "alg_bytes_per_launch": head["alg_bytes"],
                          "traffic": profiled_traffic("gemv_b1_kernel")},
             "cpu_baseline": cpu,

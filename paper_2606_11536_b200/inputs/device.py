@@ -22,8 +22,18 @@ def _load():
         lib.vipir_inputs_fill_mod.restype = ctypes.c_int
         lib.vipir_inputs_fill_mod.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64,
                                               ctypes.c_uint32, ctypes.c_void_p]
+        lib.vipir_inputs_read_only.restype = ctypes.c_int
+        lib.vipir_inputs_read_only.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p]
         _lib = lib
     return _lib
+
+
+def read_only(t):
+    """Measurement aid: stream the tensor once with plain loads, discarding the data (bench.py's
+    read-only HBM ceiling)."""
+    rc = _load().vipir_inputs_read_only(t.data_ptr(), t.numel() * t.element_size(), None, _stream())
+    if rc:
+        raise RuntimeError(f"vipir_inputs_read_only failed: {rc}")
 
 
 def _stream():
