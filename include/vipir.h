@@ -168,6 +168,17 @@ int vipir_plan_set_db_signed(vipir_plan *plan, uint32_t is_signed);
 /* Describe the plan.  Errors: INVALID_ARG. */
 int vipir_plan_info(const vipir_plan *plan, vipir_info *out);
 
+/*
+ * Introspection of the tensor-core regimes' work distribution (host only, no device needed; used by the
+ * CPU tests): the (unit, K chunk) items that group `g` of `n_groups` visits, in order, for a problem of
+ * n_units = m_tiles * n_tiles units and n_chunks chunks (csrc/gemm_i8_tcgen05.cuh "Work distribution";
+ * split = 1: the last partial round is dealt out chunk by chunk).  Writes min(*n, cap) triples
+ * (unit, chunk, must_wait) to out_triples; must_wait = 1 marks an item whose earlier chunks belong to
+ * another group.  Errors: INVALID_ARG.
+ */
+int vipir_debug_work_items(uint32_t g, uint32_t n_groups, uint32_t n_units, uint32_t n_chunks, uint32_t split,
+                           uint32_t *out_triples, uint32_t cap, uint32_t *n);
+
 /* Free the plan and its workspace.  vipir_destroy(NULL) is a no-op. */
 void vipir_destroy(vipir_plan *plan);
 

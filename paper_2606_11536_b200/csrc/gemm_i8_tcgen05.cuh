@@ -117,7 +117,7 @@ struct WorkPlan {
     uint32_t has_head, head_u, head_c0, head_c1;
 };
 
-__device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t G, uint32_t n_units, uint32_t nc,
+__host__ __device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t G, uint32_t n_units, uint32_t nc,
                                                    uint32_t split) {
     WorkPlan w;
     w.g = g; w.G = G; w.nc = nc;
@@ -150,7 +150,7 @@ __device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t G, uint3
 // f(unit, chunk, must_wait): must_wait marks the first item of a head segment -- the chunks before
 // it were (or are being) accumulated into the answer by another group.
 template <class F>
-__device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f) {
+__host__ __device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f) {
     // four segments, one loop nest (a single copy of the caller's body)
 #pragma unroll 1
     for (uint32_t seg = 0; seg < 4; ++seg) {

@@ -522,6 +522,23 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     return VIPIR_OK;
 }
 
+int vipir_debug_work_items(uint32_t g, uint32_t n_groups, uint32_t n_units, uint32_t n_chunks, uint32_t split,
+                           uint32_t* out_triples, uint32_t cap, uint32_t* n) {
+    if (!n || n_groups == 0 || g >= n_groups || n_chunks == 0 || (cap && !out_triples)) return VIPIR_ERR_INVALID_ARG;
+    const vipir::WorkPlan w = vipir::make_work_plan(g, n_groups, n_units, n_chunks, split);
+    uint32_t count = 0;
+    vipir::for_each_item(w, [&](uint32_t u, uint32_t c, bool must_wait) {
+        if (count < cap) {
+            out_triples[3 * count] = u;
+            out_triples[3 * count + 1] = c;
+            out_triples[3 * count + 2] = must_wait ? 1u : 0u;
+        }
+        ++count;
+    });
+    *n = count;
+    return VIPIR_OK;
+}
+
 void vipir_destroy(vipir_plan* p) {
     if (!p) return;
     if (p->d_planes) cudaFree(p->d_planes);

@@ -25,7 +25,7 @@ MAX_MODULI = 4
 SYMBOLS = (
     "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
     "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
-    "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
+    "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error", "vipir_debug_work_items",
     "vipir_modgemm_plan_create", "vipir_modgemm_set_h", "vipir_modgemm", "vipir_modgemm_split_c",
     "vipir_modgemm_products", "vipir_modgemm_info", "vipir_modgemm_destroy",
     "vipir_ntt_plan_create", "vipir_ntt_lift", "vipir_ntt_bad_input", "vipir_ntt_destroy",
@@ -111,6 +111,9 @@ def load() -> ctypes.CDLL:
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
         lib.vipir_destroy.argtypes = [vp]
+        lib.vipir_debug_work_items.restype = i
+        lib.vipir_debug_work_items.argtypes = [u32, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32), u32,
+                                               ctypes.POINTER(ctypes.c_uint32)]
         lib.vipir_modgemm_plan_create.restype = i
         lib.vipir_modgemm_plan_create.argtypes = [pp, u32, u64, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32)]
         lib.vipir_modgemm_set_h.restype = i
@@ -254,6 +257,16 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+def debug_work_items(g: int, n_groups: int, n_units: int, n_chunks: int, split: int = 1):
+    """vipir_debug_work_items: [(unit, chunk, must_wait), ...] for group g (host only)."""
+    cap = n_units * n_chunks + 1
+    buf = (ctypes.c_uint32 * (3 * cap))()
+    n = ctypes.c_uint32(0)
+    _check(load().vipir_debug_work_items(g, n_groups, n_units, n_chunks, split, buf, cap, ctypes.byref(n)),
+           "vipir_debug_work_items")
+    return [(buf[3 * i], buf[3 * i + 1], bool(buf[3 * i + 2])) for i in range(n.value)]
 
 
 # ---- parallel INT32 modular GEMMs  Out = H*C + (0|G) mod q_t  (include/vipir.h, NEXT-4) ----------
