@@ -117,7 +117,9 @@ int vipir_dbmul_plan_ex(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t
 
 /*
  * Enqueue answer = D * Q mod q on `cuda_stream`: the query-limb splitter
- * followed by the scan kernel of the plan's regime.  All three pointers are DEVICE pointers.
+ * followed by the scan kernel of the plan's regime -- or, for the batch-1 scan of a u8 DB whose cols
+ * are a multiple of 32, ONE kernel that splits the query words as it reads them (vipir_info.launches
+ * says which).  All three pointers are DEVICE pointers.
  * Errors: INVALID_ARG (null / misaligned pointer), CUDA.
  */
 int vipir_dbmul(vipir_plan *plan, const void *d_db, const uint32_t *d_query, uint32_t *d_answer,

@@ -15,12 +15,14 @@
 // Row sums are reduced with a transposing warp-shuffle reduction (31 shuffles for 32
 // values) and the four limb sums recombined with shifts, wrapping mod 2^32 (:249).
 //
+// With FUSED (below) the kernel takes the raw query words and splits them itself; otherwise it
 // Works on the byte view D' (rows x K' bytes, K' = cols*dl) against LC = 4 limb planes, so
 // a u16 DB with q = 2^32 runs through the same kernel (split_limbs.cuh).
 #pragma once
 #include <cstdint>
 #include <cuda.h>
 #include "ptx.cuh"
+#include "split_limbs.cuh"  // byte_transpose4 (fused query split)
 
 namespace vipir {
 
@@ -61,11 +63,17 @@ __device__ __forceinline__ uint32_t dp4a_db(uint32_t d, uint32_t q, uint32_t acc
     }
 }
 
-template <bool SIGNED>
+// FUSED: step a1 runs inside the scan.  tmL then maps the RAW query words (u8 DB only: 1024 DB bytes of a row
+// meet 1024 query words = the same 4 KiB per stage as four limb slices) as rows of 32 words, boxed 32 x 32 with
+// the 128-byte swizzle so that every thread's 64-byte run of 16 words is read with four conflict-free
+// ld.shared.v4; the thread transposes them into its four limb registers with prmt (two prmt per
+// element) -- 32 prmt next to 128 dp4a per k-step -- and the separate splitter launch disappears.
+template <bool SIGNED, bool FUSED>
 __global__ void __launch_bounds__(GV_THREADS, 1)
 gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ CUtensorMap tmL, GemvParams p) {
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    // 1024-byte alignment: the swizzled query box needs it (a stage is 36 KiB = 36 * 1024)
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * GV_STAGE_BYTES);
     uint64_t* empty = full + p.stages;
     uint32_t* red = reinterpret_cast<uint32_t*>(empty + p.stages);  // [2][GV_R]
@@ -96,8 +104,11 @@ gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ 
                     // tensor maps are typed u32: coordinates are in 4-byte elements
                     ptx::tma_load_2d(dst, &tmD, &full[stage], (int32_t)(ks * (GV_KT / 4)), (int32_t)(blk * GV_R),
                                      ptx::kEvictFirst);
-                    ptx::tma_load_2d(dst + GV_R * GV_KT, &tmL, &full[stage], (int32_t)(ks * (GV_KT / 4)), 0,
-                                     ptx::kEvictLast);
+                    if constexpr (FUSED)  // query words [ks*1024, +1024): rows ks*32 .. +32 of the 32-word view
+                        ptx::tma_load_2d(dst + GV_R * GV_KT, &tmL, &full[stage], 0, (int32_t)(ks * 32), ptx::kEvictLast);
+                    else
+                        ptx::tma_load_2d(dst + GV_R * GV_KT, &tmL, &full[stage], (int32_t)(ks * (GV_KT / 4)), 0,
+                                         ptx::kEvictLast);
                     if (++stage == p.stages) { stage = 0; phase ^= 1; }
                 }
             }
@@ -118,8 +129,22 @@ gemv_b1_kernel(const __grid_constant__ CUtensorMap tmD, const __grid_constant__ 
                 const uint8_t* sD = smem + (size_t)stage * GV_STAGE_BYTES;
                 const uint8_t* sL = sD + GV_R * GV_KT;
                 uint4 q[4];
+                if constexpr (FUSED) {
+                    // words [koff, koff + 16) of this K slice: 128-byte row koff/32, 16-byte chunks
+                    // (koff/4 % 8) + {0..3}, stored at chunk ^ (row % 8) (128B swizzle)
+                    const uint32_t row = koff >> 5, c0 = (koff >> 2) & 7;
+                    uint32_t L[4][4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) q[j] = lds128(sL + j * GV_KT + koff);
+                    for (int w = 0; w < 4; ++w) {
+                        const uint4 v = lds128(sL + row * 128 + (((c0 + w) ^ (row & 7)) << 4));
+                        byte_transpose4(v.x, v.y, v.z, v.w, L[w]);
+                    }
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) q[j] = make_uint4(L[0][j], L[1][j], L[2][j], L[3][j]);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) q[j] = lds128(sL + j * GV_KT + koff);
+                }
                 uint4 d[8];
 #pragma unroll
                 for (int rr = 0; rr < 8; ++rr) d[rr] = lds128(sD + (rw * 8 + rr) * GV_KT + koff);

@@ -104,6 +104,10 @@ struct vipir_plan {
     CUtensorMap tm_planes;
     CUtensorMap tm_db;
     const void* tm_db_for;  // d_db the cached tm_db was encoded for
+    // GEMV with the query split fused in (u8 DB, cols % 32 == 0): tensor map over the raw query words
+    bool gv_fused;
+    CUtensorMap tm_query;
+    const void* tm_query_for;
 };
 
 namespace {
@@ -269,7 +273,9 @@ int plan_gemv(vipir_plan* p) {
     g.stages = tune_env("VIPIR_TUNE_GEMV_STAGES", 4);  // 4 x 36 KiB in flight per SM measured best
     if (g.stages < 2) g.stages = 2;
     if (g.stages > 6) g.stages = 6;
-    p->smem_bytes = g.stages * vipir::GV_STAGE_BYTES + 128 + 2 * 8 * g.stages + 2 * vipir::GV_R * 4;
+    p->smem_bytes = g.stages * vipir::GV_STAGE_BYTES + 1024 + 2 * 8 * g.stages + 2 * vipir::GV_R * 4;
+    // step a1 fused into the scan when the raw query can be boxed as 32-word rows (gemv_b1.cuh "FUSED")
+    p->gv_fused = p->dl == 1 && p->cols % 32 == 0 && tune_env("VIPIR_TUNE_GEMV_FUSED", 1) != 0;
     p->grid = g.n_blocks < (uint32_t)p->num_sms ? g.n_blocks : (uint32_t)p->num_sms;
     // limb planes [4][K'] viewed as u32 elements: box 256 elements (1024 B) x 4 rows
     return make_tmap_2d(&p->tm_planes, p->d_planes, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, p->kbytes / 4, 4, p->kbytes,
@@ -394,24 +400,42 @@ int vipir_split_limbs(vipir_plan* p, const uint32_t* d_query, uint8_t* d_planes_
     return launch_split(p, d_query, d_planes_out ? d_planes_out : p->d_planes, static_cast<cudaStream_t>(cuda_stream));
 }
 
-static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaStream_t st) {
+// d_query_fused != NULL: GEMV with the query split fused in (reads the raw query instead of the limb planes)
+static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaStream_t st,
+                     const uint32_t* d_query_fused = nullptr) {
     int rc = encode_db_map(p, d_db);
     if (rc != VIPIR_OK) return rc;
     if (p->regime == VIPIR_REGIME_GEMV) {
         static thread_local bool attr_set = false;
         if (!attr_set) {
-            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)kMaxSmem));
-            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)kMaxSmem));
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)kMaxSmem));
+            CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)kMaxSmem));
             attr_set = true;
         }
         p->gv.answer = d_answer;
         p->gv.ms_bits = p->ms_bits;
-        if (p->db_signed)
-            vipir::gemv_b1_kernel<true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
-        else
-            vipir::gemv_b1_kernel<false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        if (d_query_fused) {  // raw query words, split inside the kernel
+            if (p->tm_query_for != d_query_fused) {
+                rc = make_tmap_2d(&p->tm_query, d_query_fused, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, 32, p->cols / 32, 128, 32,
+                                  32, CU_TENSOR_MAP_SWIZZLE_128B);
+                if (rc != VIPIR_OK) return rc;
+                p->tm_query_for = d_query_fused;
+            }
+            if (p->db_signed)
+                vipir::gemv_b1_kernel<true, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, p->gv);
+            else
+                vipir::gemv_b1_kernel<false, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, p->gv);
+        } else if (p->db_signed) {
+            vipir::gemv_b1_kernel<true, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        } else {
+            vipir::gemv_b1_kernel<false, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+        }
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
@@ -451,6 +475,7 @@ int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
+    if (p->regime == VIPIR_REGIME_GEMV && p->gv_fused) return scan_only(p, d_db, d_answer, st, d_query);
     int rc = launch_split(p, d_query, p->d_planes, st);
     if (rc != VIPIR_OK) return rc;
     return scan_only(p, d_db, d_answer, st);
@@ -502,7 +527,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     o->d_limb_planes = p->d_planes;
     o->modswitch_bits = p->ms_bits;
     o->db_signed = p->db_signed;
-    o->launches = (p->regime == VIPIR_REGIME_NAIVE) ? 1 : 2;
+    o->launches = (p->regime == VIPIR_REGIME_NAIVE || (p->regime == VIPIR_REGIME_GEMV && p->gv_fused)) ? 1 : 2;
     if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
         o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;
         o->n_chunks = p->gm.n_chunks;

@@ -89,6 +89,22 @@ def test_gemv_u8(rows, cols):
     check(D, Q, None, G)
 
 
+@pytest.mark.parametrize("fused", ["1", "0"])
+@pytest.mark.parametrize("signed,bits", [(False, 0), (True, 0), (False, 18)])
+def test_gemv_fused_and_separate_split_agree_with_the_oracle(fused, signed, bits, monkeypatch):
+    """cols % 32 == 0: the query split runs inside the scan kernel (one launch); VIPIR_TUNE_GEMV_FUSED=0
+    forces the two-launch path.  Ragged rows, a K tail shorter than a stage, several stages."""
+    monkeypatch.setenv("VIPIR_TUNE_GEMV_FUSED", fused)
+    rows, cols = 1000, 1024 * 5 + 32 * 7
+    D, Q = make(77, rows, cols, 1)
+    got, info = run_dbmul(D, Q, None, G, return_info=True, modswitch_bits=bits, db_signed=signed)
+    assert info["launches"] == (1 if fused == "1" else 2)
+    want = oracle.dbmul_signed(D, Q, None) if signed else oracle.dbmul(D, Q, None, nthreads=NT)
+    if bits:
+        want = oracle.modswitch(want, bits)
+    assert_same(got, want)
+
+
 def test_gemv_u16_wrapping():
     D, Q = make(43, 70, 520, 1, 16)
     check(D, Q, None, G)
@@ -287,6 +303,8 @@ def test_mma_prime_edges(regime):
 def test_auto_regime_choice():
     ensure_built()
     with vipir.Plan(1024, 1024, 1) as p:
+        assert p.info["regime_name"] == "gemv" and p.info["launches"] == 1     # query split fused into the scan
+    with vipir.Plan(1024, 1040, 1) as p:                                     # cols % 32 != 0: separate splitter
         assert p.info["regime_name"] == "gemv" and p.info["launches"] == 2
     with vipir.Plan(1024, 1024, 8) as p:
         assert p.info["regime_name"] == "mma_1sm" and p.info["mma_n"] == 32
