@@ -74,6 +74,14 @@ typedef enum {
     VIPIR_REGIME_NAIVE = 4
 } vipir_regime;
 
+/* Layout of the database in device memory.  ROW_MAJOR: rows x cols
+ * elements, u8 or little-endian u16, as the caller holds it.  LIMB_PLANES (u16 only; BASELINE.json
+ * configs[4]: "uint16 ... (split into 2 u8 limbs)"): the two byte matrices D_lo[r][k] = D[r][k] & 0xFF
+ * and D_hi[r][k] = D[r][k] >> 8, each rows x cols u8 row-major, D_hi directly behind D_lo
+ * (2*rows*cols bytes) -- written once, offline, by vipir_db_split_u16; the DB of a PIR server is
+ * static and resident in GPU DRAM, prepared like the hint. */
+typedef enum { VIPIR_DB_ROW_MAJOR = 0, VIPIR_DB_LIMB_PLANES = 1 } vipir_db_layout;
+
 typedef struct {
     uint32_t regime;          /* the regime in effect (never AUTO) */
     uint32_t db_limbs;        /* dl: 1 (u8) or 2 (u16) */
@@ -94,7 +102,9 @@ typedef struct {
     void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
     uint32_t modswitch_bits;  /* fused output modulus switch in effect (0 = off) */
     uint32_t db_signed;       /* 1 if the DB elements are read as two's-complement int8 (vipir_plan_set_db_signed) */
-    uint32_t m_sub;           /* MMA regimes: 128-row DB sub-tiles per CTA and tile (rows per tile = 128 * CTAs * m_sub) */
+    uint32_t m_sub;           /* MMA regimes: 128-row DB sub-tiles per CTA and tile (rows per tile = 128 * CTAs * m_sub;
+                                 LIMB_PLANES: the two limb tiles of a row block count as two sub-tiles) */
+    uint32_t db_layout;       /* vipir_db_layout the plan expects d_db in */
 } vipir_info;
 
 /*
@@ -114,6 +124,28 @@ int vipir_dbmul_plan(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t ba
  * (GEMV needs T*batch == 1 and q = 2^32). */
 int vipir_dbmul_plan_ex(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
                         const vipir_modulus_spec *mod, uint32_t regime);
+
+/*
+ * Same, for a database held in `db_layout` (vipir_db_layout).  With VIPIR_DB_LIMB_PLANES the d_db
+ * passed to vipir_dbmul / vipir_dbmul_scan / vipir_dbmul_host is the buffer vipir_db_split_u16
+ * wrote; the answer is that of the u16 database it was made from, bit for bit.  The tensor-core
+ * kernel then runs 8 int8 MACs per u16 x u32 product (two DB limbs x four query limbs)
+ * against four limb-plane columns per query vector, instead of the 10 and 5 of the byte view of an
+ * interleaved u16 row (DESIGN.md sections 5, 14).
+ * Errors: as vipir_dbmul_plan_ex; INVALID_ARG (unknown layout); UNSUPPORTED (LIMB_PLANES with
+ * db_bits != 16, with the GEMV or NAIVE regime, with cols % 16 != 0, or with rows >= 2^30).
+ */
+int vipir_dbmul_plan_layout(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                            const vipir_modulus_spec *mod, uint32_t regime, uint32_t db_layout);
+
+/*
+ * Offline, once per database: de-interleave a u16 DB (rows x cols, row-major, little-endian) into
+ * the VIPIR_DB_LIMB_PLANES form.  d_db_u16, d_db_planes: DEVICE pointers, 16-byte aligned,
+ * 2*rows*cols bytes each, caller-owned, not overlapping.  Enqueues one kernel on `cuda_stream`.
+ * Errors: INVALID_ARG (null / misaligned / overlapping pointers, zero sizes), UNSUPPORTED
+ * (cols % 16 != 0, rows or cols >= 2^31), CUDA.
+ */
+int vipir_db_split_u16(const void *d_db_u16, void *d_db_planes, uint64_t rows, uint64_t cols, void *cuda_stream);
 
 /*
  * Enqueue answer = D * Q mod q on `cuda_stream`: the query-limb splitter

@@ -31,6 +31,13 @@
 // sub-tiles per k-atom against ONE limb-tile box: msub accumulators side by side in TMEM, the
 // limb-plane traffic per DB byte divided by msub.
 //
+// Limb-plane u16 DB (NL = 2): a u16 DB that was de-interleaved once, offline,
+// into its two byte matrices [D_lo ; D_hi] (vipir_db_split_u16) is scanned as the u8 matrix of 2*rows
+// rows it then is: the two limb tiles of the same 128 rows are two of the CTA's M sub-tiles (msub is a
+// multiple of 2), their accumulators sit side by side in TMEM, and the epilogue thread that owns the
+// row adds them as  P_lo + 2^8 P_hi  before the one reduction.  8 int8 MACs per u16 x u32 product and
+// 4 limb-plane columns per query vector instead of the byte view's 10 and 5.
+//
 // Work distribution.  A work item is (unit = (M tile, N tile), K chunk).  Groups (a CTA, or a
 // CTA pair) take whole units round-robin for the full rounds -- so that the sibling N tiles of
 // one M tile run at the same time on neighbouring groups and share the DB tile through L2 --
@@ -73,7 +80,7 @@ struct GemmParams {
     uint32_t stages;
     uint32_t stage_bytes;    // per CTA = katoms * atom_bytes
     uint32_t tmem_cols, acc_stages;
-    uint32_t msub;           // 128-row DB sub-tiles per CTA and unit (1, 2 or 4): rows per unit = 128 * CG * msub
+    uint32_t msub;           // 128-row DB sub-tiles per CTA and unit (1, 2 or 4): rows per unit = 128 * CG * msub / NL
     uint32_t split;          // deal the last, partial round out chunk by chunk (1) or unit by unit (0)
     uint32_t n_groups;       // CTAs (CG = 1) or CTA pairs (CG = 2) launched
     uint32_t* sync;          // [0] ticket, [1] groups finished, [2 + i] epilogue-warp arrivals of leftover unit i
@@ -175,7 +182,9 @@ __host__ __device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f)
 
 #pragma nv_diag_default 20013
 
-template <int CG, int LC, bool PRIME>
+// NL = byte-limb planes of the DB held as separate matrices (1: u8 DB or the byte view of a u16 DB;
+// 2: limb-plane u16 DB, D_hi starting p.rows rows below D_lo in the tensor map).
+template <int CG, int LC, bool PRIME, int NL = 1>
 __global__ void __launch_bounds__(GM_THREADS, 1)
 gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, GemmParams p) {
     extern __shared__ uint8_t smem_raw[];
@@ -193,6 +202,8 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
     const uint32_t n_units = p.m_tiles * p.n_tiles;
     const uint32_t acc_cols = p.msub * p.bn;  // TMEM columns of one accumulator stage
+    const uint32_t rsub = p.msub / NL;         // 128*CG-row blocks per unit
+    static_assert(NL == 1 || (NL == 2 && LC == 4), "limb-plane DBs use the four plain query limb planes");
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmA);
@@ -243,8 +254,11 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
             for_each_item(work, [&](uint32_t u, uint32_t c, bool) {
                 const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
-                // sub-tile j of the unit = rows [(mt*msub + j) * 128*CG, +128*CG); this CTA's 128 of them
-                const int32_t row0 = (int32_t)((mt * p.msub * CG + rank) * GM_BM);
+                // sub-tile j of the unit = limb plane j % NL of rows [(mt*rsub + j/NL) * 128*CG, +128*CG);
+                // this CTA's 128 of them
+                auto sub_row = [&](uint32_t j) {
+                    return (int32_t)((j % NL) * p.rows + ((uint64_t)(mt * rsub + j / NL) * CG + rank) * GM_BM);
+                };
                 const uint32_t ks_begin = c * p.ksteps_per_chunk;
                 const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
                 // a stage never straddles a chunk: the last stage of a chunk may hold fewer atoms
@@ -268,15 +282,13 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         const int32_t k0 = (int32_t)((ks0 + a) * GM_BK);
                         if constexpr (CG == 1) {
                             for (uint32_t j = 0; j < p.msub; ++j)
-                                ptx::tma_load_2d(sA + j * GM_A_BYTES, &tmA, &full[stage], k0,
-                                                 row0 + (int32_t)(j * GM_BM), hintA);
+                                ptx::tma_load_2d(sA + j * GM_A_BYTES, &tmA, &full[stage], k0, sub_row(j), hintA);
                             for (uint32_t j = 0; j < p.n_instr; ++j)
                                 ptx::tma_load_2d(sB + j * b_bytes, &tmB, &full[stage], k0,
                                                  (int32_t)(nt * p.bn + j * p.ni_cols), ptx::kEvictLast);
                         } else {
                             for (uint32_t j = 0; j < p.msub; ++j)
-                                ptx::tma_load_2d_pair(sA + j * GM_A_BYTES, &tmA, bar, k0,
-                                                      row0 + (int32_t)(j * 2 * GM_BM), hintA);
+                                ptx::tma_load_2d_pair(sA + j * GM_A_BYTES, &tmA, bar, k0, sub_row(j), hintA);
                             for (uint32_t j = 0; j < p.n_instr; ++j)
                                 ptx::tma_load_2d_pair(sB + j * b_bytes, &tmB, bar, k0,
                                                       (int32_t)(nt * p.bn + j * p.ni_cols + rank * b_rows),
@@ -374,10 +386,10 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             constexpr uint32_t kPf = 8;
             const bool ms_final = !PRIME && p.ms_bits != 0 && c + 1 == p.n_chunks;
             const bool need_old = c > 0 && (PRIME || ms_final);
-            for (uint32_t m = 0; m < p.msub; ++m) {
-                const uint64_t row = (uint64_t)((mt * p.msub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
+            for (uint32_t m = 0; m < rsub; ++m) {
+                const uint64_t row = (uint64_t)((mt * rsub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
                 const bool row_ok = row < p.rows;
-                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols + m * p.bn;
+                const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols + m * NL * p.bn;
                 for (uint32_t g0 = 0; g0 < p.qt / 4; g0 += kPf) {
                     uint32_t old[4 * kPf];
                     if (need_old) {
@@ -395,6 +407,8 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         uint32_t v[4 * LC];
                         ptx::tmem_ld16(tacc + g * (4 * LC), v);
                         if constexpr (LC == 5) ptx::tmem_ld4(tacc + g * (4 * LC) + 16, v + 16);
+                        uint32_t w[NL == 2 ? 4 * LC : 1];  // the D_hi sub-tile's sums for the same row
+                        if constexpr (NL == 2) ptx::tmem_ld16(tacc + p.bn + g * (4 * LC), w);
                         ptx::tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
@@ -405,6 +419,8 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                     // shifts, wrap mod 2^32 (an s = 4 column would vanish)
                                     uint32_t val =
                                         v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
+                                    if constexpr (NL == 2)  // D = D_lo + 2^8 D_hi; the 2^32 term of w[3] vanishes
+                                        val += (w[i * LC] << 8) + (w[i * LC + 1] << 16) + (w[i * LC + 2] << 24);
                                     if (ms_final) {
                                         if (c > 0) val += old[gg * 4 + i];
                                         *dst = modswitch_word(val, p.ms_bits);
@@ -417,7 +433,14 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                     const uint32_t t = q / p.batch;
                                     const uint32_t pm = p.moduli[t];
                                     uint32_t val;
-                                    if constexpr (LC == 4) {
+                                    if constexpr (NL == 2) {
+                                        // unsigned; each sum < 2^31, so x < 2^63.1
+                                        uint64_t x = 0;
+#pragma unroll
+                                        for (int s = 0; s < LC; ++s)
+                                            x += ((uint64_t)v[i * LC + s] + ((uint64_t)w[i * LC + s] << 8)) << (8 * s);
+                                        val = barrett_u64(x, pm, p.barrett[t]);
+                                    } else if constexpr (LC == 4) {
                                         // every |P_s| < 2^31 (R7), so the s32 reading is exact for u8 and s8
                                         // DBs alike and |x| < 2^56; a negative x reduces as p - (|x| mod p)
                                         int64_t x = 0;

@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/vipir.h"
+#include "db_split.cuh"
 #include "gemm_i8_tcgen05.cuh"
 #include "gemv_b1.cuh"
 #include "naive.cuh"
@@ -84,6 +85,8 @@ uint32_t ceil_div(uint32_t x, uint32_t m) { return (x + m - 1) / m; }
 struct vipir_plan {
     uint64_t rows, cols, kbytes;
     uint32_t batch, db_bits, dl, lc, nq, n_moduli;
+    uint32_t db_layout;  // VIPIR_DB_ROW_MAJOR or VIPIR_DB_LIMB_PLANES (u16 only)
+    uint32_t kdl;        // DB bytes per k in one row of the matrix the kernels scan: dl, or 1 for limb planes
     uint32_t moduli[VIPIR_MAX_MODULI];
     uint32_t regime;
     uint32_t ms_bits;  // fused modulus switch (0 = off)
@@ -112,9 +115,9 @@ struct vipir_plan {
 
 namespace {
 
-template <int CG, int LC, bool PRIME>
+template <int CG, int LC, bool PRIME, int NL = 1>
 int launch_gemm(vipir_plan* p, cudaStream_t st) {
-    auto kern = vipir::gemm_i8_kernel<CG, LC, PRIME>;
+    auto kern = vipir::gemm_i8_kernel<CG, LC, PRIME, NL>;
     static thread_local bool attr_set = false;
     if (!attr_set) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
@@ -139,6 +142,8 @@ int launch_gemm(vipir_plan* p, cudaStream_t st) {
 template <int CG>
 int launch_gemm_cg(vipir_plan* p, cudaStream_t st) {
     const bool prime = p->n_moduli > 0;
+    if (p->db_layout == VIPIR_DB_LIMB_PLANES)
+        return prime ? launch_gemm<CG, 4, true, 2>(p, st) : launch_gemm<CG, 4, false, 2>(p, st);
     if (p->lc == 5) return launch_gemm<CG, 5, true>(p, st);
     return prime ? launch_gemm<CG, 4, true>(p, st) : launch_gemm<CG, 4, false>(p, st);
 }
@@ -146,7 +151,7 @@ int launch_gemm_cg(vipir_plan* p, cudaStream_t st) {
 int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaStream_t st) {
     const uint64_t groups = ((p->cols + 15) / 16) * p->nq;
     const uint32_t blocks = (uint32_t)((groups + 255) / 256);
-    if (p->dl == 1)
+    if (p->kdl == 1)
         vipir::split_limbs_kernel<1, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
     else if (p->lc == 4)
         vipir::split_limbs_kernel<2, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
@@ -162,7 +167,9 @@ int plan_gemm(vipir_plan* p, int cg) {
     vipir::GemmParams& g = p->gm;
     memset(&g, 0, sizeof g);
     const uint32_t lc = p->lc;
-    const uint32_t bn_max = (cg == 1) ? 256u : 512u;
+    // limb-plane u16 DB: the two limb tiles of a row block are two M sub-tiles, so msub >= 2
+    const uint32_t nl = (p->db_layout == VIPIR_DB_LIMB_PLANES) ? 2u : 1u;
+    const uint32_t bn_max = (cg == 1 || nl == 2) ? 256u : 512u;
     const uint32_t q_align = (lc == 5) ? 16u : 4u;       // keeps bn a multiple of 16 and of 4*LC
     const uint32_t q_align2 = (lc == 5) ? 32u : 8u;      // two instructions: bn/2 a multiple of 16
     const uint32_t qt_max = (bn_max / lc) / q_align2 * q_align2;
@@ -191,15 +198,20 @@ int plan_gemm(vipir_plan* p, int cg) {
     g.total_ksteps = (uint32_t)((p->kbytes + vipir::GM_BK - 1) / vipir::GM_BK);
     const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
     g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
+    {
+        const uint32_t min_chunks = tune_env("VIPIR_TUNE_MIN_CHUNKS", 0);
+        if (min_chunks > g.n_chunks && min_chunks <= g.total_ksteps) g.n_chunks = min_chunks;
+    }
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
     const uint32_t max_groups = (uint32_t)p->num_sms / cg;
     // M sub-tiles per CTA (gemm_i8_tcgen05.cuh): while the product is HBM-bound every DB byte drags
     // bn / (128 * cg * msub) limb-plane bytes through L2 -> SM with it, and that fill (~8 TB/s on the
     // whole chip) is what caps the scan; so take the most sub-tiles that keep two accumulator stages
     // in TMEM, three pipeline stages in shared memory and >= 2 work items per group.
-    uint32_t msub = 1;
-    for (uint32_t cand = 4; cand > 1; cand >>= 1) {
-        const uint64_t units = (p->rows + 128ull * cg * cand - 1) / (128ull * cg * cand) * g.n_tiles;
+    uint32_t msub = nl;
+    for (uint32_t cand = 4; cand > nl; cand >>= 1) {
+        const uint64_t rows_unit = 128ull * cg * (cand / nl);
+        const uint64_t units = (p->rows + rows_unit - 1) / rows_unit * g.n_tiles;
         const uint32_t atom = cand * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
         if (2 * cand * bn <= 512 && 3 * atom <= kMaxSmem - 1280 && units * g.n_chunks >= 2ull * max_groups) {
             msub = cand;
@@ -207,9 +219,11 @@ int plan_gemm(vipir_plan* p, int cg) {
         }
     }
     const uint32_t msub_force = tune_env("VIPIR_TUNE_MSUB", 0);
-    if ((msub_force == 1 || msub_force == 2 || msub_force == 4) && msub_force * bn <= 512) msub = msub_force;
+    if ((msub_force == 1 || msub_force == 2 || msub_force == 4) && msub_force * bn <= 512 && msub_force % nl == 0)
+        msub = msub_force;
     g.msub = msub;
-    g.m_tiles = (uint32_t)((p->rows + 128ull * cg * msub - 1) / (128ull * cg * msub));
+    const uint64_t rows_unit = 128ull * cg * (msub / nl);
+    g.m_tiles = (uint32_t)((p->rows + rows_unit - 1) / rows_unit);
     g.atom_bytes = msub * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
     const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
     // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes"); VIPIR_TUNE_* override
@@ -289,7 +303,9 @@ int encode_db_map(vipir_plan* p, const void* d_db) {
         rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, p->kbytes / 4, p->rows, p->kbytes,
                           vipir::GV_KT / 4, vipir::GV_R, CU_TENSOR_MAP_SWIZZLE_NONE);
     else
-        rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes, p->rows, p->kbytes,
+        // limb planes: D_hi lies directly behind D_lo, one u8 matrix of 2*rows rows
+        rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes,
+                          p->rows * (p->db_layout == VIPIR_DB_LIMB_PLANES ? 2 : 1), p->kbytes,
                           vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B,
                           (CUtensorMapL2promotion)tune_env("VIPIR_TUNE_L2PROMO", CU_TENSOR_MAP_L2_PROMOTION_L2_256B));
     if (rc == VIPIR_OK) p->tm_db_for = d_db;
@@ -316,21 +332,33 @@ const char* vipir_last_cuda_error(void) { return g_cuda_err; }
 
 int vipir_dbmul_plan_ex(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
                         const vipir_modulus_spec* mod, uint32_t regime) {
+    return vipir_dbmul_plan_layout(out, rows, cols, batch, db_bits, mod, regime, VIPIR_DB_ROW_MAJOR);
+}
+
+int vipir_dbmul_plan_layout(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                            const vipir_modulus_spec* mod, uint32_t regime, uint32_t db_layout) {
     if (!out) return VIPIR_ERR_INVALID_ARG;
     *out = nullptr;
     // ---- argument checks first: these need no device ----
     if (rows == 0 || cols == 0 || batch == 0) return VIPIR_ERR_INVALID_ARG;
     if (db_bits != 8 && db_bits != 16) return VIPIR_ERR_INVALID_ARG;
     if (regime > VIPIR_REGIME_NAIVE) return VIPIR_ERR_INVALID_ARG;
+    if (db_layout > VIPIR_DB_LIMB_PLANES) return VIPIR_ERR_INVALID_ARG;
+    const bool planes = db_layout == VIPIR_DB_LIMB_PLANES;
+    // limb planes exist for u16 DBs and are scanned by the tensor-core regimes only
+    if (planes && (db_bits != 16 || regime == VIPIR_REGIME_GEMV || regime == VIPIR_REGIME_NAIVE))
+        return VIPIR_ERR_UNSUPPORTED;
     const uint32_t n_moduli = mod ? mod->count : 0;
     if (n_moduli > VIPIR_MAX_MODULI) return VIPIR_ERR_INVALID_ARG;
     if (n_moduli > 0 && !mod->moduli) return VIPIR_ERR_INVALID_ARG;
     for (uint32_t t = 0; t < n_moduli; ++t)
         if (mod->moduli[t] < 2 || mod->moduli[t] >= (1u << 30)) return VIPIR_ERR_INVALID_ARG;
     const uint32_t dl = db_bits / 8;
-    if (cols > (1ull << 31) || (cols * dl) % 16 != 0) return VIPIR_ERR_UNSUPPORTED;
-    const uint64_t kbytes = cols * dl;
+    const uint32_t kdl = planes ? 1u : dl;
+    if (cols > (1ull << 31) || (cols * kdl) % 16 != 0) return VIPIR_ERR_UNSUPPORTED;
+    const uint64_t kbytes = cols * kdl;
     if (rows >= (1ull << 31) || kbytes >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    if (planes && rows >= (1ull << 30)) return VIPIR_ERR_UNSUPPORTED;  // 2*rows rows in one tensor map
     const uint32_t T = n_moduli ? n_moduli : 1;
     if ((uint64_t)T * batch * 5 >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
 
@@ -352,14 +380,16 @@ int vipir_dbmul_plan_ex(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t
     p->batch = batch;
     p->db_bits = db_bits;
     p->dl = dl;
+    p->kdl = kdl;
+    p->db_layout = db_layout;
     p->n_moduli = n_moduli;
     for (uint32_t t = 0; t < n_moduli; ++t) p->moduli[t] = mod->moduli[t];
     p->nq = T * batch;
-    p->lc = (dl == 2 && n_moduli > 0) ? 5u : 4u;  // split_limbs.cuh: the s = 4 column vanishes mod 2^32
+    p->lc = (kdl == 2 && n_moduli > 0) ? 5u : 4u;  // split_limbs.cuh: the s = 4 column vanishes mod 2^32
     p->num_sms = sms;
 
     if (regime == VIPIR_REGIME_AUTO) {
-        if (p->nq == 1 && n_moduli == 0) regime = VIPIR_REGIME_GEMV;
+        if (p->nq == 1 && n_moduli == 0 && !planes) regime = VIPIR_REGIME_GEMV;
         // measured (profiles/r01_tuning.md): CTA pairs win from 32 query vectors up, where the limb
         // tile's shared-memory traffic starts to matter; below that one CTA per tile is as fast
         else regime = ((uint64_t)p->nq * p->lc > 64 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
@@ -499,6 +529,24 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     return VIPIR_OK;
 }
 
+int vipir_db_split_u16(const void* d_db_u16, void* d_db_planes, uint64_t rows, uint64_t cols, void* cuda_stream) {
+    if (!d_db_u16 || !d_db_planes || rows == 0 || cols == 0) return VIPIR_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_db_u16) & 15) || (reinterpret_cast<uintptr_t>(d_db_planes) & 15))
+        return VIPIR_ERR_INVALID_ARG;
+    if (cols % 16 != 0 || rows >= (1ull << 31) || cols >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    const uint64_t bytes = rows * cols * 2;
+    const uintptr_t a = reinterpret_cast<uintptr_t>(d_db_u16), b = reinterpret_cast<uintptr_t>(d_db_planes);
+    if (a < b + bytes && b < a + bytes) return VIPIR_ERR_INVALID_ARG;  // not in place
+    const uint64_t n16 = rows * cols / 16;
+    const uint64_t want = (n16 + 255) / 256;
+    const uint32_t blocks = (uint32_t)(want < 148ull * 32 ? want : 148ull * 32);
+    uint8_t* lo = static_cast<uint8_t*>(d_db_planes);
+    vipir::db_split_u16_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        static_cast<const uint4*>(d_db_u16), reinterpret_cast<uint4*>(lo), reinterpret_cast<uint4*>(lo + rows * cols), n16);
+    CK(cudaGetLastError());
+    return VIPIR_OK;
+}
+
 int vipir_plan_set_modswitch(vipir_plan* p, uint32_t out_bits) {
     if (!p || out_bits > 31) return VIPIR_ERR_INVALID_ARG;
     if (out_bits != 0 && (p->n_moduli != 0 || p->regime == VIPIR_REGIME_NAIVE)) return VIPIR_ERR_UNSUPPORTED;
@@ -527,6 +575,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     o->d_limb_planes = p->d_planes;
     o->modswitch_bits = p->ms_bits;
     o->db_signed = p->db_signed;
+    o->db_layout = p->db_layout;
     o->launches = (p->regime == VIPIR_REGIME_NAIVE || (p->regime == VIPIR_REGIME_GEMV && p->gv_fused)) ? 1 : 2;
     if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
         o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;

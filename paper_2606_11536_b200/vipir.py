@@ -19,11 +19,12 @@ _lib = None
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_ARCH = range(6)
 REGIME_AUTO, REGIME_GEMV, REGIME_MMA_1SM, REGIME_MMA_2SM, REGIME_NAIVE = range(5)
 REGIME_NAMES = {0: "auto", 1: "gemv", 2: "mma_1sm", 3: "mma_2sm", 4: "naive"}
+DB_ROW_MAJOR, DB_LIMB_PLANES = 0, 1
 MAX_MODULI = 4
 
 # every symbol include/vipir.h declares
 SYMBOLS = (
-    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
+    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul_plan_layout", "vipir_db_split_u16", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
     "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error", "vipir_debug_work_items",
     "vipir_modgemm_plan_create", "vipir_modgemm_set_h", "vipir_modgemm", "vipir_modgemm_split_c",
@@ -45,6 +46,7 @@ class Info(ctypes.Structure):
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
         ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
         ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32), ("m_sub", ctypes.c_uint32),
+        ("db_layout", ctypes.c_uint32),
     ]
 
     def as_dict(self):
@@ -95,6 +97,10 @@ def load() -> ctypes.CDLL:
         lib.vipir_dbmul_plan.argtypes = [pp, u64, u64, u32, u32, ms]
         lib.vipir_dbmul_plan_ex.restype = i
         lib.vipir_dbmul_plan_ex.argtypes = [pp, u64, u64, u32, u32, ms, u32]
+        lib.vipir_dbmul_plan_layout.restype = i
+        lib.vipir_dbmul_plan_layout.argtypes = [pp, u64, u64, u32, u32, ms, u32, u32]
+        lib.vipir_db_split_u16.restype = i
+        lib.vipir_db_split_u16.argtypes = [vp, vp, u64, u64, vp]
         lib.vipir_dbmul.restype = i
         lib.vipir_dbmul.argtypes = [vp, vp, vp, vp, vp]
         lib.vipir_dbmul_host.restype = i
@@ -168,8 +174,9 @@ def _ptr(t):
     return ctypes.c_void_p(t.ctypes.data)
 
 
-def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, regime: int = REGIME_AUTO):
-    """vipir_dbmul_plan[_ex]; returns the opaque plan handle (a c_void_p)."""
+def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, regime: int = REGIME_AUTO,
+               db_layout: int = DB_ROW_MAJOR):
+    """vipir_dbmul_plan[_ex|_layout]; returns the opaque plan handle (a c_void_p)."""
     lib = load()
     handle = ctypes.c_void_p()
     spec_p = None
@@ -177,8 +184,15 @@ def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, 
         arr = (ctypes.c_uint32 * len(moduli))(*[int(m) for m in moduli])
         spec = ModulusSpec(len(moduli), arr)
         spec_p = ctypes.byref(spec)
-    _check(lib.vipir_dbmul_plan_ex(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime), "vipir_dbmul_plan")
+    _check(lib.vipir_dbmul_plan_layout(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime, db_layout),
+           "vipir_dbmul_plan")
     return handle
+
+
+def db_split_u16(d_db_u16, d_db_planes, rows: int, cols: int, stream=None):
+    """vipir_db_split_u16: offline de-interleave of a u16 DB into its two byte-limb planes."""
+    _check(load().vipir_db_split_u16(_ptr(d_db_u16), _ptr(d_db_planes), rows, cols, _stream_ptr(stream)),
+           "vipir_db_split_u16")
 
 
 def dbmul(plan, d_db, d_query, d_answer, stream=None):
@@ -227,8 +241,8 @@ class Plan:
     """Context-manager convenience around dbmul_plan / destroy."""
 
     def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO, modswitch_bits=0,
-                 db_signed=False):
-        self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime)
+                 db_signed=False, db_layout=DB_ROW_MAJOR):
+        self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime, db_layout)
         if modswitch_bits:
             plan_set_modswitch(self.handle, modswitch_bits)
         if db_signed:

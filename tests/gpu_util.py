@@ -11,8 +11,9 @@ def ensure_built():
 
 
 def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.REGIME_AUTO, return_info=False,
-              modswitch_bits=0, db_signed=False):
-    """D_host rows x cols (u8/u16), Q_host [T][B][cols] u32 -> answer [T][B][rows] u32 via libvipir."""
+              modswitch_bits=0, db_signed=False, db_layout=vipir.DB_ROW_MAJOR):
+    """D_host rows x cols (u8/u16), Q_host [T][B][cols] u32 -> answer [T][B][rows] u32 via libvipir.
+    db_layout = DB_LIMB_PLANES: the u16 DB is first re-laid out on the device by vipir_db_split_u16."""
     import torch
     ensure_built()
     D_host = np.ascontiguousarray(D_host)
@@ -23,7 +24,11 @@ def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.
     d_db = torch.from_numpy(D_host.view(np.uint8).reshape(rows, -1)).cuda()
     d_q = torch.from_numpy(Q_host.view(np.int32)).cuda()
     d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")  # poison
-    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits, db_signed) as plan:
+    if db_layout == vipir.DB_LIMB_PLANES:
+        d_planes = torch.full_like(d_db, 0x5A)
+        vipir.db_split_u16(d_db, d_planes, rows, cols)
+        d_db = d_planes
+    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits, db_signed, db_layout) as plan:
         plan(d_db, d_q, d_a)
         torch.cuda.synchronize()
         info = plan.info

@@ -20,7 +20,7 @@ def lib():
 def test_header_symbols_are_exported(lib):
     header = (ROOT / "include" / "vipir.h").read_text()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)  # declarations only, not comments
-    declared = set(re.findall(r"\b(vipir_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(vipir_[a-z0-9_]+)\s*\(", header))
     assert declared == set(vipir.SYMBOLS), declared ^ set(vipir.SYMBOLS)
     for name in declared:
         assert hasattr(lib, name), name
@@ -85,6 +85,27 @@ def test_null_out_pointer(lib):
     assert lib.vipir_dbmul_scan(None, None, None, None) == vipir.ERR_INVALID_ARG
     assert lib.vipir_plan_set_modswitch(None, 18) == vipir.ERR_INVALID_ARG
     assert lib.vipir_plan_set_db_signed(None, 1) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_dbmul_plan_layout(None, 16, 16, 1, 16, None, 0, 1) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_db_split_u16(None, None, 16, 16, None) == vipir.ERR_INVALID_ARG
+
+
+def test_limb_plane_layout_argument_checks(lib):
+    """VIPIR_DB_LIMB_PLANES: u16 only, tensor-core regimes only, cols % 16 == 0, 2*rows < 2^31 --
+    all rejected before any device call."""
+    def st(rows, cols, batch, db_bits, regime, layout):
+        h = ctypes.c_void_p()
+        return lib.vipir_dbmul_plan_layout(ctypes.byref(h), rows, cols, batch, db_bits, None, regime, layout)
+    assert st(64, 32, 1, 16, 0, 2) == vipir.ERR_INVALID_ARG
+    assert st(64, 32, 1, 8, 0, 1) == vipir.ERR_UNSUPPORTED
+    assert st(64, 32, 1, 16, vipir.REGIME_GEMV, 1) == vipir.ERR_UNSUPPORTED
+    assert st(64, 32, 1, 16, vipir.REGIME_NAIVE, 1) == vipir.ERR_UNSUPPORTED
+    assert st(64, 24, 1, 16, 0, 1) == vipir.ERR_UNSUPPORTED
+    assert st(1 << 30, 32, 1, 16, 0, 1) == vipir.ERR_UNSUPPORTED
+    one = ctypes.c_void_p(0x1000)
+    assert lib.vipir_db_split_u16(one, ctypes.c_void_p(0x100000), 0, 16, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_db_split_u16(one, ctypes.c_void_p(0x100000), 16, 24, None) == vipir.ERR_UNSUPPORTED
+    assert lib.vipir_db_split_u16(ctypes.c_void_p(0x1001), ctypes.c_void_p(0x100000), 16, 16, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_db_split_u16(one, ctypes.c_void_p(0x1100), 16, 16, None) == vipir.ERR_INVALID_ARG  # overlap
 
 
 def test_no_silent_fallback_without_a_gpu(lib):

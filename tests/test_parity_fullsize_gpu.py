@@ -56,7 +56,7 @@ def sample_rows(rows, n_random=24):
     return sorted(set(r for r in fixed + rnd if 0 <= r < rows))
 
 
-def run(name, device_db):
+def run(name, device_db, limb_planes=False):
     import torch
     from paper_2606_11536_b200.inputs import device
     rows, cols, batch, db_bits, moduli, regime = CONFIGS[name]
@@ -65,9 +65,13 @@ def run(name, device_db):
     d_q = device.query(SEED, cols, batch, moduli)
     T = d_q.shape[0]
     d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")
-    with vipir.Plan(rows, cols, batch, db_bits, moduli) as plan:
+    d_scan, layout = d_db, vipir.DB_ROW_MAJOR
+    if limb_planes:  # the u16 DB re-laid out once into its two byte-limb planes (vipir_db_split_u16)
+        d_scan, layout = torch.empty_like(d_db), vipir.DB_LIMB_PLANES
+        vipir.db_split_u16(d_db, d_scan, rows, cols)
+    with vipir.Plan(rows, cols, batch, db_bits, moduli, db_layout=layout) as plan:
         assert plan.info["regime_name"] == regime
-        plan(d_db, d_q, d_a)
+        plan(d_scan, d_q, d_a)
         torch.cuda.synchronize()
     return d_db, d_q, d_a
 
@@ -122,6 +126,15 @@ def test_config2_full_compare(device_db):
 @pytest.mark.parametrize("name", ["C3_16GiB_B1", "C3_16GiB_B8", "C4_4GiB_B256", "C5_rns_u16_B64"])
 def test_fullsize_sampled_rows_and_column_sums(name, device_db):
     d_db, d_q, d_a = run(name, device_db)
+    check_sampled_rows(name, d_a)
+    check_column_sum_identity(name, d_db, d_a)
+
+
+def test_config5_limb_plane_layout(device_db):
+    """configs[4] with the u16 DB held as its two byte-limb planes (bench.py: C5_rns_u16_B64x2_planes):
+    same answer as the u16 definition -- sampled rows, every word canonical, column sums over all rows."""
+    name = "C5_rns_u16_B64"
+    d_db, d_q, d_a = run(name, device_db, limb_planes=True)
     check_sampled_rows(name, d_a)
     check_column_sum_identity(name, d_db, d_a)
 
