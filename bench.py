@@ -459,7 +459,8 @@ def run_cuda(args):
     extra = {}
     cpu = None
     if rank == 0 and world == 1:
-        for name in ([BATCHED] if not args.all else [n for n in CONFIGS if n != HEADLINE]):
+        # every BASELINE.json config rides along at N = 1 (a few seconds); --headline-only keeps just configs[2] and [3]
+        for name in ([BATCHED] if args.headline_only else [n for n in CONFIGS if n != HEADLINE]):
             tensor_bound = name in (BATCHED, "C5_rns_u16_B64x2", "C5_rns_u16_B64x2_planes")
             extra[name] = run_config(name, buf, args.steps, max(3, args.warmup), peaks,
                                      settle_s=1.0 if tensor_bound else 0.0)
@@ -527,7 +528,7 @@ def run_cuda(args):
             line["ntt"] = extra.pop("ntt")
         if "pipeline" in extra:
             line["pipeline"] = extra.pop("pipeline")
-        if args.all or args.paper:
+        if extra:
             line["configs"] = {n: {k: v for k, v in r.items() if k not in ("alg_bytes", "int8_ops")} for n, r in extra.items()}
             line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in ("alg_bytes", "int8_ops")}
         print(json.dumps(line))
@@ -577,7 +578,8 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--all", action="store_true", help="also time every other BASELINE.json config")
+    ap.add_argument("--all", action="store_true", help="(default since r01j) time every BASELINE.json config at N = 1")
+    ap.add_argument("--headline-only", action="store_true", help="time only configs[2] (headline) and configs[3] (batched)")
     ap.add_argument("--paper", action="store_true", help="also time the paper's Table-2 shapes and NEXT-2 shapes (64 GiB DB)")
     ap.add_argument("--modgemm", action="store_true",
                     help="also time the ring-packing stage at the paper's 64 GiB shape: lift + NTT (G, H) and H*C+(0|G)")
