@@ -81,6 +81,7 @@ struct GemmParams {
     uint32_t stage_bytes;    // per CTA = katoms * atom_bytes
     uint32_t tmem_cols, acc_stages;
     uint32_t msub;           // 128-row DB sub-tiles per CTA and unit (1, 2 or 4): rows per unit = 128 * CG * msub / NL
+    uint32_t collector;      // n_instr == 2: second N half reuses the A operand from the collector buffer
     uint32_t split;          // deal the last, partial round out chunk by chunk (1) or unit by unit (0)
     uint32_t n_groups;       // CTAs (CG = 1) or CTA pairs (CG = 2) launched
     uint32_t* sync;          // [0] ticket, [1] groups finished, [2 + i] epilogue-warp arrivals of leftover unit i
@@ -331,6 +332,20 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         const uint32_t accumulate = (ks0 + a > ks_begin) ? 1u : 0u;
                         for (uint32_t m = 0; m < p.msub; ++m) {
                             const uint64_t dA = make_smem_desc(sA + m * GM_A_BYTES);
+                            if (p.n_instr == 2 && p.collector) {
+                                // two N halves against the same DB slice: issue them back to back and let
+                                // the second take A from the collector instead of shared memory
+                                const uint64_t dB0 = make_smem_desc(sB), dB1 = make_smem_desc(sB + b_bytes);
+#pragma unroll
+                                for (uint32_t kk = 0; kk < GM_BK / GM_UMMA_K; ++kk) {
+                                    const uint64_t koff = (uint64_t)((kk * GM_UMMA_K) >> 4);
+                                    const uint32_t acc = (accumulate || kk > 0) ? 1u : 0u;
+                                    ptx::mma_i8_collect<CG, 1>(tacc + m * p.bn, dA + koff, dB0 + koff, p.idesc, acc);
+                                    ptx::mma_i8_collect<CG, 2>(tacc + m * p.bn + p.ni_cols, dA + koff, dB1 + koff, p.idesc,
+                                                               acc);
+                                }
+                                continue;
+                            }
                             for (uint32_t j = 0; j < p.n_instr; ++j) {
                                 const uint64_t dB = make_smem_desc(sB + j * b_bytes);
 #pragma unroll

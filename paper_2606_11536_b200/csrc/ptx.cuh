@@ -224,6 +224,29 @@ __device__ __forceinline__ void tc_fence_after() {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 }
 
+// Same with a collector hint for the A operand: KEEP = 1 keeps A in the tensor core's collector buffer
+// after this MMA (.collector::a::fill), KEEP = 2 takes A from the collector, where the previous MMA --
+// same A descriptor -- left it, instead of re-reading shared memory (.collector::a::lastuse).
+template <int CG, int KEEP>
+__device__ __forceinline__ void mma_i8_collect(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                               uint32_t accumulate) {
+    static_assert(KEEP == 1 || KEEP == 2, "fill or lastuse");
+#define VIPIR_MMA_I8_COLLECT(cg, usage)                                                                \
+    asm volatile(                                                                                      \
+        "{\n\t"                                                                                        \
+        ".reg .pred p;\n\t"                                                                            \
+        "setp.ne.b32 p, %4, 0;\n\t"                                                                    \
+        "tcgen05.mma.cta_group::" cg ".kind::i8.collector::a::" usage " [%0], %1, %2, %3, p;\n\t"      \
+        "}\n" ::"r"(tmem_d),                                                                           \
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)                                          \
+        : "memory")
+    if constexpr (CG == 1 && KEEP == 1) VIPIR_MMA_I8_COLLECT("1", "fill");
+    if constexpr (CG == 1 && KEEP == 2) VIPIR_MMA_I8_COLLECT("1", "lastuse");
+    if constexpr (CG == 2 && KEEP == 1) VIPIR_MMA_I8_COLLECT("2", "fill");
+    if constexpr (CG == 2 && KEEP == 2) VIPIR_MMA_I8_COLLECT("2", "lastuse");
+#undef VIPIR_MMA_I8_COLLECT
+}
+
 // D[tmem] (+)= A[smem] * B[smem], 8-bit integer operands, s32 accumulators.
 template <int CG>
 __device__ __forceinline__ void mma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,

@@ -258,6 +258,7 @@ int plan_gemm(vipir_plan* p, int cg) {
     // groups: one per SM (pair); fewer only when there are fewer work items (unit, K chunk) than that
     const uint64_t items = (uint64_t)g.m_tiles * g.n_tiles * g.n_chunks;
     g.split = tune_env("VIPIR_TUNE_SPLIT", 1);
+    g.collector = tune_env("VIPIR_TUNE_COLLECTOR", 1);
     const uint64_t n_units64 = (uint64_t)g.m_tiles * g.n_tiles;
     g.n_groups = (uint32_t)(items < max_groups ? items : max_groups);
     if (!g.split && n_units64 < g.n_groups) g.n_groups = (uint32_t)n_units64;
