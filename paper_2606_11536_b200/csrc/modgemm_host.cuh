@@ -127,10 +127,9 @@ int plan_modgemm(vipir_modgemm_plan* p) {
 template <int CG>
 int launch_modgemm(vipir_modgemm_plan* p, cudaStream_t st) {
     auto kern = vipir::modgemm_i8_kernel<CG>;
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
+    static thread_local uint64_t attr_set = 0;  // bit d: done on device d
+    if (attr_needed(attr_set)) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        attr_set = true;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p->grid);

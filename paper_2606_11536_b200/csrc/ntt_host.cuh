@@ -42,10 +42,9 @@ int launch_ntt(vipir_ntt_plan* p, const vipir::NttParams& np, cudaStream_t st) {
     constexpr uint32_t STR = N + N / 16 + 4;
     const uint32_t smem = ((TW_SMEM ? 2 * N : 0) + P * STR) * sizeof(uint32_t);
     auto kern = vipir::ntt_lift_kernel<L, NT, R, TW_SMEM, MINB>;
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
+    static thread_local uint64_t attr_set = 0;  // bit d: done on device d
+    if (attr_needed(attr_set)) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        attr_set = true;
     }
     const uint64_t groups = (uint64_t)np.n_outer * ((np.n_inner + P - 1) / P);
     const uint64_t cap = (uint64_t)p->num_sms * (BIG ? 1 : 4);

@@ -30,6 +30,16 @@ int cuda_fail(cudaError_t e, const char* where) {
     } while (0)
 
 uint32_t tune_env(const char* name, uint32_t dflt);
+// the opt-in shared-memory attribute of a kernel is per device: true the first time the calling thread
+// asks on the current device
+bool attr_needed(uint64_t& done_mask) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return true;
+    const uint64_t bit = 1ull << (dev & 63);
+    if (done_mask & bit) return false;
+    done_mask |= bit;
+    return true;
+}
 constexpr uint32_t kMaxSmem = 232448;  // 227 KiB opt-in dynamic shared memory per CTA
 constexpr uint32_t kChunkBytes = 32768; // 255*255*32768 < 2^31 (R7)
 
@@ -118,10 +128,9 @@ namespace {
 template <int CG, int LC, bool PRIME, int NL = 1>
 int launch_gemm(vipir_plan* p, cudaStream_t st) {
     auto kern = vipir::gemm_i8_kernel<CG, LC, PRIME, NL>;
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
+    static thread_local uint64_t attr_set = 0;  // bit d: done on device d
+    if (attr_needed(attr_set)) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        attr_set = true;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p->grid);
@@ -437,8 +446,8 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
     int rc = encode_db_map(p, d_db);
     if (rc != VIPIR_OK) return rc;
     if (p->regime == VIPIR_REGIME_GEMV) {
-        static thread_local bool attr_set = false;
-        if (!attr_set) {
+        static thread_local uint64_t attr_set = 0;  // bit d: done on device d
+        if (attr_needed(attr_set)) {
             CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)kMaxSmem));
             CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -447,7 +456,6 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
                                     (int)kMaxSmem));
             CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)kMaxSmem));
-            attr_set = true;
         }
         p->gv.answer = d_answer;
         p->gv.ms_bits = p->ms_bits;
