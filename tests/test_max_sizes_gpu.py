@@ -27,12 +27,13 @@ PRIMES = inputs.rns_primes(0)
 
 def _need_memory(gb):
     import torch
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < gb * (1 << 30):
         pytest.skip(f"needs {gb} GiB of free device memory, {free >> 30} GiB available")
 
 
-@pytest.mark.parametrize("batch,moduli,regime", [(1, None, "gemv"), (2, None, "mma_1sm"), (1, [PRIMES[0]], "mma_1sm")])
+@pytest.mark.parametrize("batch,moduli,regime", [(1, None, "gemv"), (2, [PRIMES[0]], "mma_1sm")])
 def test_maximum_rows(batch, moduli, regime):
     import torch
     from paper_2606_11536_b200.inputs import device
