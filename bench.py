@@ -173,6 +173,20 @@ def time_events(fn, steps, warmup, stream):
     return e0.elapsed_time(e1)  # ms for `steps` calls
 
 
+def step_spread(fn, steps, stream):
+    """Median and best single-step time (an event after every step; SURVEY.md 8(d) asks for both).  Reported beside the
+    K-step total, which stays the value's basis."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for i in range(steps):
+        fn()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    t = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(steps))
+    return {"median": t[len(t) // 2], "best": t[0], "worst": t[-1]}
+
+
 def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset_bytes=0, settle_s=0.0):
     """Times one config on the current device; returns a dict of measurements."""
     import torch
@@ -203,6 +217,8 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
                     plan(d_db, d_q, d_a)
                 torch.cuda.synchronize()
         ms_step = time_events(lambda: plan(d_db, d_q, d_a), steps, warmup, stream) / steps
+        if with_e2e:  # headline config: spread of the single steps as well
+            out["ms_step_spread"] = step_spread(lambda: plan(d_db, d_q, d_a), min(steps, 50), stream)
         # the dominant kernel alone (planes already in the workspace) and the splitter alone
         if info["launches"] == 1:   # GEMV with the split fused in: the step IS the scan kernel (same timed region)
             ms_scan = ms_step
@@ -397,7 +413,12 @@ def cpu_baseline(sample_rows: int, device_db, cols: int):
         dt = time.perf_counter() - t0
         if passes >= 3 and dt >= 1.0:
             break
+    # one thread, on the first 1024 rows (128 MiB) of the same sample (single- and all-thread times)
+    t1 = time.perf_counter()
+    oracle.dbmul(D[:1024], Q, nthreads=1)
+    dt1 = time.perf_counter() - t1
     return {"value": passes * D.size / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "single_thread_GBps": D[:1024].size / dt1 / 1e9,
             "sample": f"{passes} passes over the first {sample_rows} of 131072 rows x 131072 cols, batch 1 "
                       f"({D.size / 2**30:.0f} GiB of DB per pass), {dt:.2f} s wall on {cores} threads "
                       f"= {dt * cores:.0f} core-seconds", "seconds": dt}, A
@@ -498,6 +519,7 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": head["h2d_bytes"],
                     "d2h_bytes_per_step": head["d2h_bytes"], "ms_per_step": head["e2e_ms"]},
             "gpu_launches": head["plan"]["launches"] * args.steps,
+            "ms_per_step_spread": head.get("ms_step_spread"),
             "roofline": {"bound": "hbm", "kernel": "gemv_b1_kernel", "achieved": head["scan_kernel_GBps"],
                          "peak": peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)"
                          if peaks["source"] == "measured" else "fallback 6650 GB/s (B200_PROFILING.md)",
