@@ -208,12 +208,8 @@ int plan_gemm(vipir_plan* p, int cg) {
     const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
     g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
     {
-        // a short K (one chunk) with few M tiles leaves pairs idle in the last round and nothing to deal out chunk by
-        // chunk: cut K into 8 pieces anyway (measured: 1 GiB DB, 32 queries, 5.1 -> 5.4 TB/s; profiles/r01_tuning.md)
-        const uint64_t units2 = (p->rows + 128ull * cg * 2 - 1) / (128ull * cg * 2) * g.n_tiles;
-        uint32_t min_chunks = (cg == 2 && nl == 1 && g.n_chunks == 1 && g.total_ksteps >= 128 && units2 < 2ull * ((uint32_t)p->num_sms / cg))
-                                  ? 8u : 0u;
-        min_chunks = tune_env("VIPIR_TUNE_MIN_CHUNKS", min_chunks);
+        // experiments: finer work items for short K (profiles/r01_tuning.md section 6: no robust gain, not a rule)
+        const uint32_t min_chunks = tune_env("VIPIR_TUNE_MIN_CHUNKS", 0);
         if (min_chunks > g.n_chunks && min_chunks <= g.total_ksteps) g.n_chunks = min_chunks;
     }
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
