@@ -163,7 +163,9 @@ int vipir_dbmul(vipir_plan *plan, const void *d_db, const uint32_t *d_query, uin
  * PAPER.md:176).  Copies h_query to the device, runs vipir_dbmul, copies the answer back and
  * waits for the stream.  h_query / h_answer: HOST pointers with the d_query / d_answer
  * layouts (pinned memory makes the copies asynchronous); d_db: DEVICE pointer.  The first
- * call allocates device staging owned by the plan.
+ * call allocates device staging owned by the plan.  When h_answer is pinned, device-mapped host memory
+ * (cudaHostAlloc / cudaHostRegister) the batch-1 scan stores the answer into it directly and no
+ * device-to-host copy is made; the result is complete when the call returns either way.
  */
 int vipir_dbmul_host(vipir_plan *plan, const void *d_db, const uint32_t *h_query, uint32_t *h_answer,
                      void *cuda_stream);

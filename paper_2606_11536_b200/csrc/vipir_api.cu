@@ -532,6 +532,20 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
         }
     }
     CK(cudaMemcpyAsync(p->d_q_stage, h_query, qbytes, cudaMemcpyHostToDevice, st));
+    // batch-1 scan into pinned, device-mapped host memory: the kernel's plain 128-byte answer stores go straight
+    // over PCIe while the scan runs, and the device-to-host copy after it disappears.  (The tensor-core regimes
+    // read-modify-write the answer between K chunks and keep the staging buffer.)
+    if (p->regime == VIPIR_REGIME_GEMV && tune_env("VIPIR_TUNE_HOST_DIRECT", 1)) {
+        cudaPointerAttributes attr{};
+        if (cudaPointerGetAttributes(&attr, h_answer) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
+            attr.devicePointer != nullptr) {
+            int rc = vipir_dbmul(p, d_db, p->d_q_stage, static_cast<uint32_t*>(attr.devicePointer), cuda_stream);
+            if (rc != VIPIR_OK) return rc;
+            CK(cudaStreamSynchronize(st));
+            return VIPIR_OK;
+        }
+        cudaGetLastError();  // not a CUDA-known pointer: pageable memory, fall through to the staged copy
+    }
     int rc = vipir_dbmul(p, d_db, p->d_q_stage, p->d_a_stage, cuda_stream);
     if (rc != VIPIR_OK) return rc;
     CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
