@@ -22,7 +22,8 @@
  * Layouts (all dense, no pitch):
  *   d_db      rows x cols, row-major (cols contiguous), uint8, or little-endian uint16 when
  *             db_bits == 16.  DEVICE pointer, 16-byte aligned.  cols * db_bits/8 must be a
- *             multiple of 16 bytes.
+ *             multiple of 16 bytes.  (A uint16 database may instead be handed over as its two
+ *             byte-limb planes, prepared once by vipir_db_split_u16: vipir_db_layout below.)
  *   d_query   [T][batch][cols] uint32 -- each query vector contiguous.  DEVICE pointer, 16-byte aligned.
  *   d_answer  [T][batch][rows] uint32.  DEVICE pointer.
  * Ownership: the caller owns d_db, d_query, d_answer (they must not overlap and must stay
