@@ -159,3 +159,44 @@ def test_ntt_plan_argument_checks(lib):
     import torch
     if not torch.cuda.is_available():     # a valid request must fail loudly without a B200, never succeed
         assert _ntt_status(lib, 1, 4, [q], [psi16], [1], 6) in (vipir.ERR_CUDA, vipir.ERR_ARCH)
+
+
+def test_header_is_plain_c_and_links_from_c(lib, tmp_path):
+    """include/vipir.h compiles as strict C99 and a C program linked against libvipir.so (no Python, no
+    torch) reaches the entry points: status strings, argument errors before any device call."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "abi.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include <string.h>
+#include "vipir.h"
+int main(void) {
+    vipir_plan *plan = (vipir_plan *)1;
+    vipir_modulus_spec spec;
+    uint32_t bad = 1u << 30;
+    vipir_info info;
+    spec.count = 1; spec.moduli = &bad;
+    if (strcmp(vipir_status_str(VIPIR_OK), "VIPIR_OK")) return 1;
+    if (vipir_dbmul_plan(&plan, 0, 16, 1, 8, NULL) != VIPIR_ERR_INVALID_ARG || plan != NULL) return 2;
+    if (vipir_dbmul_plan(&plan, 16, 16, 1, 8, &spec) != VIPIR_ERR_INVALID_ARG) return 3;
+    if (vipir_dbmul_plan_layout(&plan, 16, 16, 1, 8, NULL, VIPIR_REGIME_AUTO, VIPIR_DB_LIMB_PLANES) != VIPIR_ERR_UNSUPPORTED) return 4;
+    if (vipir_dbmul(NULL, NULL, NULL, NULL, NULL) != VIPIR_ERR_INVALID_ARG) return 5;
+    if (vipir_plan_info(NULL, &info) != VIPIR_ERR_INVALID_ARG) return 6;
+    if (vipir_db_split_u16(NULL, NULL, 1, 16, NULL) != VIPIR_ERR_INVALID_ARG) return 7;
+    vipir_destroy(NULL);
+    vipir_modgemm_destroy(NULL);
+    vipir_ntt_destroy(NULL);
+    puts("c abi ok");
+    return 0;
+}
+''')
+    so = vipir.lib_path()
+    exe = tmp_path / "abi"
+    subprocess.run([gcc, "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", "-I", str(ROOT / "include"), str(src),
+                    "-o", str(exe), str(so), f"-Wl,-rpath,{so.parent}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    assert "c abi ok" in out
