@@ -156,3 +156,34 @@ def test_limb_planes_host_entry_point_and_plan_reuse():
             h_a = torch.full((2, batch, rows), -1, dtype=torch.int32).pin_memory()
             plan.host(d_db, h_q, h_a)
             assert_same(h_a.numpy().view(np.uint32), oracle.dbmul(D, Q, PRIMES, nthreads=NT))
+
+
+def _random_cases(n, seed):
+    g = np.random.default_rng(seed)
+    cases = []
+    for _ in range(n):
+        rows = int(g.integers(1, 900))
+        cols = int(g.integers(1, 300)) * 16
+        if g.random() < 0.2:
+            cols += 32768 * int(g.integers(1, 3))              # cross one or two K-chunk seams
+            rows = int(g.integers(1, 300))
+        kind = g.random()
+        moduli = None if kind < 0.35 else [int(g.integers(2, 1 << 30)) for _ in range(int(g.integers(1, 5)))]
+        batch = int(g.choice([1, 2, 3, 5, 8, 17, 33, 64, 70, 130]))
+        if cols > 40000:
+            batch = min(batch, 8)
+        regime = int(g.choice([AUTO, M1, M2]))
+        cases.append((rows, cols, batch, moduli, regime))
+    return cases
+
+
+@pytest.mark.parametrize("case", _random_cases(30, 2025),
+                         ids=lambda c: f"{c[0]}x{c[1]}xB{c[2]}m{0 if c[3] is None else len(c[3])}r{c[4]}")
+def test_random_shapes_limb_planes(case):
+    rows, cols, batch, moduli, regime = case
+    D = inputs.db_rows(rows * 31 + cols, rows, cols, 16)
+    Q = inputs.query(rows * 31 + cols, cols, batch, moduli)
+    if moduli is None:
+        Q[0, 0, : min(cols, 5)] = 0xFFFFFFFF
+    got = run_dbmul(D, Q, moduli, regime, db_layout=LP)
+    assert_same(got, oracle.dbmul(D, Q, moduli, nthreads=NT))
