@@ -59,6 +59,10 @@ PAPER_CONFIGS = {
     "P_16GiB_B32": (131072, 131072, 32, 8, False),
     "P_64GiB_B32": (262144, 262144, 32, 8, False),
     "P_64GiB_B1": (262144, 262144, 1, 8, False),
+    # throughput against batch size at a fixed DB (the paper's Fig 6 sweeps B = 1..32; B = 1, 8, 32 are above)
+    "F6_16GiB_B2": (131072, 131072, 2, 8, False),
+    "F6_16GiB_B4": (131072, 131072, 4, 8, False),
+    "F6_16GiB_B16": (131072, 131072, 16, 8, False),
     "N2_hint_4GiB_B1280": (65536, 65536, 1280, 8, False),
     "N2_tall_64GiB_B1": (1 << 20, 65536, 1, 8, False),
     # DoublePIR / double-packing second folding, one client: (8N x D1) INT8 by D1 x (n+1) INT32
