@@ -86,9 +86,9 @@ typedef enum { VIPIR_DB_ROW_MAJOR = 0, VIPIR_DB_LIMB_PLANES = 1 } vipir_db_layou
 typedef struct {
     uint32_t regime;          /* the regime in effect (never AUTO) */
     uint32_t db_limbs;        /* dl: 1 (u8) or 2 (u16) */
-    uint32_t limb_cols;       /* LC: accumulator columns per query vector (4, or 5 for u16 + prime) */
+    uint32_t limb_cols;       /* LC: accumulator columns per query vector (4; 5 for a row-major u16 DB with prime moduli) */
     uint32_t query_vectors;   /* T * batch */
-    uint64_t k_bytes;         /* K' = cols * dl: bytes per DB row */
+    uint64_t k_bytes;         /* K' = cols * dl: bytes per DB row (LIMB_PLANES: cols, the bytes per row of one limb plane) */
     uint32_t k_chunk_bytes;   /* K' bytes per int32 accumulation chunk (<= 32768); 0 for GEMV/NAIVE */
     uint32_t n_chunks;
     uint32_t tile_queries;    /* query vectors per N tile (MMA regimes) */
