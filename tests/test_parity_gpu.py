@@ -344,6 +344,38 @@ def test_plan_reuse_with_new_buffers_and_host_entry_point():
         assert_same(h_a.numpy().view(np.uint32), oracle.dbmul(D, Q))
 
 
+@pytest.mark.parametrize("bits", [0, 18])
+def test_host_entry_point_batch1_pinned_and_pageable(bits):
+    """vipir_dbmul_host at batch 1: into pinned (device-mapped) host memory the scan kernel stores the answer
+    directly, into pageable memory it goes through the staged copy -- same words either way, also at an
+    unaligned offset inside a pinned buffer and with the fused modulus switch."""
+    import torch
+    ensure_built()
+    rows, cols = 1000, 2080
+    D, Q = make(88, rows, cols, 1)
+    want = oracle.dbmul(D, Q, nthreads=NT)
+    if bits:
+        want = oracle.modswitch(want, bits)
+    d_db = torch.from_numpy(D).cuda()
+    h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+    with vipir.Plan(rows, cols, 1, modswitch_bits=bits) as plan:
+        assert plan.info["regime_name"] == "gemv"
+        pinned = torch.full((rows + 7,), -1, dtype=torch.int32).pin_memory()
+        for off in (0, 3):
+            pinned.fill_(-1)
+            h_a = pinned[off:off + rows]
+            plan.host(d_db, h_q, h_a)
+            assert_same(h_a.numpy().view(np.uint32).reshape(1, 1, rows), want)
+            assert (pinned[:off] == -1).all() and (pinned[off + rows:] == -1).all()
+        pageable = torch.full((1, 1, rows), -1, dtype=torch.int32)
+        plan.host(d_db, h_q, pageable)
+        assert_same(pageable.numpy().view(np.uint32), want)
+        pageable_q = torch.from_numpy(Q.view(np.int32).copy())
+        pinned.fill_(-1)
+        plan.host(d_db, pageable_q, pinned[:rows])
+        assert_same(pinned[:rows].numpy().view(np.uint32).reshape(1, 1, rows), want)
+
+
 def test_misaligned_pointers_are_rejected():
     import torch
     ensure_built()
