@@ -50,6 +50,25 @@ def test_ntt_matches_oracle(log2n, n_a, M, layout, centered):
     assert np.array_equal(got, want), f"{(got != want).sum()} of {got.size} words differ"
 
 
+@pytest.mark.parametrize("which", ["below_2^29", "above_2^29", "mixed"])
+def test_ntt_prime_ranges_adversarial(which):
+    """Primes below 2^29 (the paper's) and just below 2^30 (the ABI's limit: the lazy butterflies keep
+    values in [0, 4q) < 2^32) -- adversarial inputs (all words p - 1, scale q - 1) next to random ones, N = 2^12."""
+    N, log2n, p_bits = 4096, 12, 18
+    big = inputs.rns_primes(0, 2, 1 << 30, 8192)           # just below 2^30, = 1 mod 2N
+    assert all(q > (1 << 29) for q in big)
+    moduli = {"below_2^29": Q29, "above_2^29": big, "mixed": [Q29[0], big[0]]}[which]
+    psi = [oracle.smallest_psi(N, q) for q in moduli]
+    scale = [q - 1 for q in moduli]
+    g = np.random.default_rng(7)
+    X = g.integers(0, 1 << p_bits, size=(2, 3 * N), dtype=np.uint32)
+    X[1, :N] = (1 << p_bits) - 1
+    for centered in (False, True):
+        got, bad = run_ntt(X, log2n, moduli, psi, scale, p_bits, centered, vipir.NTT_LAYOUT_G)
+        want = oracle.ntt_lift(X, N, moduli, psi, scale, p_bits, centered, vipir.NTT_LAYOUT_G, nthreads=16)
+        assert not bad and np.array_equal(got, want), f"{(got != want).sum()} of {got.size} words differ"
+
+
 def test_ntt_monomials_and_bad_input_flag():
     N, log2n, p_bits = 4096, 12, 18
     psi = [oracle.smallest_psi(N, q) for q in Q29]
