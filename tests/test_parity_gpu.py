@@ -156,6 +156,25 @@ def test_mma_large_batch_two_n_tiles(regime):
     assert_same(got, oracle.dbmul(D, Q, None, nthreads=NT))
 
 
+@pytest.mark.parametrize("regime,cols", [(AUTO, 65536), (M2, 65536 - 112)])
+def test_mma_config4_launch_path_compared_in_full(regime, cols):
+    """The exact launch path of BASELINE.json configs[3] (four limbs, int32 accumulation per K
+    chunk, shift-recombine, free wrap), every answer word compared: q = 2^32 with no fused modulus switch, CTA
+    pairs, B = 256 = two N tiles of 512 accumulator columns, TWO tcgen05.mma per K slice (the second taking the
+    DB operand from the collector), two K chunks -- chunk 0 stores, chunk 1 accumulates with red.global.add.
+    Rows: 2 full 256-row pair tiles + 88 ragged rows; K: configs[3]'s own 65536 columns = two full 32768-byte
+    chunks, and 65424 columns = the same two chunks with a 16-byte tail in the last k-step."""
+    rows, batch = 600, 256
+    D, Q = make(53, rows, cols, batch)
+    D[:3] = 255                            # int32 accumulators at 255 * 255 * 32768 on a few rows
+    Q[0, :2, :] = 0xFFFFFFFF
+    got, info = run_dbmul(D, Q, None, regime, return_info=True)
+    assert info["regime_name"] == "mma_2sm" and info["modswitch_bits"] == 0
+    assert info["tile_cols"] == 512 and info["mma_n"] * 2 == info["tile_cols"]  # n_instr == 2
+    assert info["n_tiles"] == 2 and info["n_chunks"] == 2 and info["k_chunk_bytes"] <= 32768
+    assert_same(got, oracle.dbmul(D, Q, None, nthreads=NT))
+
+
 # ---- M sub-tiles and chunk-granular work distribution (gemm_i8_tcgen05.cuh header) ---------------
 
 @pytest.mark.parametrize("regime", [M1, M2])
