@@ -99,8 +99,7 @@ typedef struct {
     uint32_t smem_bytes;      /* dynamic shared memory per CTA */
     uint32_t grid;            /* CTAs launched by the main kernel */
     uint32_t launches;        /* kernels enqueued per vipir_dbmul call */
-    uint64_t workspace_bytes; /* limb planes */
-    void *d_limb_planes;      /* DEVICE pointer to the planes [query_vectors*LC][K'] u8 (read-only for callers; tests) */
+    uint64_t workspace_bytes; /* limb planes [query_vectors*LC][K'] u8, owned by the plan */
     uint32_t modswitch_bits;  /* fused output modulus switch in effect (0 = off) */
     uint32_t db_signed;       /* 1 if the DB elements are read as two's-complement int8 (vipir_plan_set_db_signed) */
     uint32_t m_sub;           /* MMA regimes: 128-row DB sub-tiles per CTA and tile (rows per tile = 128 * CTAs * m_sub;
@@ -138,6 +137,33 @@ int vipir_dbmul_plan_ex(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t
  */
 int vipir_dbmul_plan_layout(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
                             const vipir_modulus_spec *mod, uint32_t regime, uint32_t db_layout);
+
+/*
+ * Explicit planner overrides (DESIGN.md section 6 "Regimes" and "M sub-tiles"): every field 0 = the planner's own
+ * choice, so a zeroed struct (or tune == NULL) is vipir_dbmul_plan_layout.  They select between code paths that
+ * all compute the same, bit-exact answer -- for tests that must reach each path and for measurements; nothing
+ * in the library reads the environment.  A value outside a field's domain is INVALID_ARG; a value the shape or
+ * regime cannot honour (for example m_sub * tile_cols > 512 TMEM columns) is UNSUPPORTED -- never silently ignored.
+ */
+typedef struct {
+    uint32_t m_sub;          /* MMA: 128-row DB sub-tiles per CTA and tile: 1, 2 or 4 */
+    uint32_t tile_queries;   /* MMA: query vectors per N tile (a multiple of 4; of 16 when limb_cols == 5), <= 128 */
+    uint32_t k_atoms;        /* MMA: 128-byte k-atoms per pipeline stage, 1..8 (lowered until two stages fit) */
+    uint32_t stages;         /* shared-memory ring depth: MMA 2..12 (at most what fits), GEMV 2..6 */
+    uint32_t min_chunks;     /* MMA: cut K into at least this many chunks (finer work items; <= number of k-atoms) */
+    uint32_t separate_split; /* GEMV: 1 = always run the query-limb splitter as its own kernel (two launches) */
+    uint32_t whole_units;    /* MMA: 1 = deal the last, partial round of work units out whole, not chunk by chunk */
+    uint32_t no_collector;   /* MMA: 1 = the second N half re-reads the DB operand from shared memory */
+    uint32_t host_staged;    /* vipir_dbmul_host: 1 = always stage the answer in device memory and copy it back
+                                (no direct stores into mapped host memory, no overlapped copies) */
+    uint32_t reserved[7];    /* must be 0 */
+} vipir_tuning;
+
+/* vipir_dbmul_plan_layout with explicit planner overrides.  Errors: as vipir_dbmul_plan_layout; INVALID_ARG
+ * (a field outside its domain, reserved != 0); UNSUPPORTED (an override this shape / regime cannot honour). */
+int vipir_dbmul_plan_tuned(vipir_plan **out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                           const vipir_modulus_spec *mod, uint32_t regime, uint32_t db_layout,
+                           const vipir_tuning *tune);
 
 /*
  * Offline, once per database: de-interleave a u16 DB (rows x cols, row-major, little-endian) into
@@ -205,17 +231,6 @@ int vipir_plan_set_db_signed(vipir_plan *plan, uint32_t is_signed);
 /* Describe the plan.  Errors: INVALID_ARG. */
 int vipir_plan_info(const vipir_plan *plan, vipir_info *out);
 
-/*
- * Introspection of the tensor-core regimes' work distribution (host only, no device needed; used by the
- * CPU tests): the (unit, K chunk) items that group `g` of `n_groups` visits, in order, for a problem of
- * n_units = m_tiles * n_tiles units and n_chunks chunks (csrc/gemm_i8_tcgen05.cuh "Work distribution";
- * split = 1: the last partial round is dealt out chunk by chunk).  Writes min(*n, cap) triples
- * (unit, chunk, must_wait) to out_triples; must_wait = 1 marks an item whose earlier chunks belong to
- * another group.  Errors: INVALID_ARG.
- */
-int vipir_debug_work_items(uint32_t g, uint32_t n_groups, uint32_t n_units, uint32_t n_chunks, uint32_t split,
-                           uint32_t *out_triples, uint32_t cap, uint32_t *n);
-
 /* Free the plan and its workspace.  vipir_destroy(NULL) is a no-op. */
 void vipir_destroy(vipir_plan *plan);
 
@@ -269,10 +284,17 @@ typedef struct {
     uint32_t a_stages, b_stages, acc_stages;
     uint32_t smem_bytes, grid;
     uint32_t launches;      /* kernels enqueued per vipir_modgemm call */
-    uint64_t h_limb_bytes, c_limb_bytes;
-    void *d_h_limbs;        /* DEVICE: [T*NC*M][4*Kp] u8, byte (k/128)*512 + i*128 + k%128 of a row = limb i of H[..][k] */
-    void *d_c_limbs;        /* DEVICE: [T*NC][4][ncols][Kp] u8 */
+    uint64_t h_limb_bytes, c_limb_bytes; /* plan-owned workspaces: H limbs [T*NC*M][4*Kp] u8, C limbs [T*NC][4][ncols][Kp] u8 */
 } vipir_modgemm_info_t;
+
+/* Explicit planner overrides for the modular GEMMs; every field 0 = the planner's own choice (see vipir_tuning). */
+typedef struct {
+    uint32_t cta_group;   /* 1, or 2 = CTA pairs */
+    uint32_t tile_cols;   /* ct: columns of C per N tile, a multiple of 8, <= 64 */
+    uint32_t a_stages;    /* ring depth of the H operand: 4..24 (at most what fits) */
+    uint32_t b_stages;    /* ring depth of the C operand: 2..4 */
+    uint32_t reserved[4]; /* must be 0 */
+} vipir_modgemm_tuning;
 
 /*
  * Build a plan (host; allocates the limb workspaces on the current device).
@@ -282,6 +304,12 @@ typedef struct {
  */
 int vipir_modgemm_plan_create(vipir_modgemm_plan **out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K,
                               uint32_t ncols, uint32_t gcols, const uint32_t *moduli);
+
+/* Same with explicit planner overrides.  Errors: as above; INVALID_ARG (a field outside its domain),
+ * UNSUPPORTED (an override the shape cannot honour). */
+int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan **out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K,
+                                    uint32_t ncols, uint32_t gcols, const uint32_t *moduli,
+                                    const vipir_modgemm_tuning *tune);
 
 /* OFFLINE step: split the static hint H into byte limbs in the plan's GEMM-friendly layout (the
  * paper's "layout transposition before the GEMMs"; H is precomputed offline,

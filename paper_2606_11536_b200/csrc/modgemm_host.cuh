@@ -1,6 +1,6 @@
 // modgemm_host.cuh -- host side (plan, dispatch, C ABI) of the parallel INT32 modular GEMMs
 // Out = H*C + (0|G) mod q_t (include/vipir.h "vipir_modgemm_*"; kernels in modgemm_i8.cuh).
-// Textually included at the end of vipir_api.cu: it uses that file's helpers (CK, tune_env,
+// Textually included at the end of vipir_api.cu: it uses that file's helpers (CK,
 // get_encode_fn, g_cuda_err).
 #pragma once
 #include "modgemm_i8.cuh"
@@ -9,6 +9,7 @@ struct vipir_modgemm_plan {
     uint32_t T, M, K, Kp, ncols, gcols, cg;
     uint64_t NC, P;
     uint32_t moduli[VIPIR_MAX_MODULI];
+    vipir_modgemm_tuning tune;  // explicit planner overrides; all zero = the planner's own choices
     int num_sms;
     uint8_t* d_hp;       // H byte limbs, interleaved per k-atom: [P*M][4*Kp]   (written by vipir_modgemm_set_h)
     uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
@@ -62,8 +63,7 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         n_tiles = ceil_div(p->ncols, 64);
         ct = round_up(ceil_div(p->ncols, n_tiles), 8);
     }
-    const uint32_t ct_force = tune_env("VIPIR_TUNE_MG_CT", 0);
-    if (ct_force >= 8 && ct_force <= 64 && ct_force % 8 == 0) {
+    if (const uint32_t ct_force = p->tune.tile_cols) {
         ct = ct_force;
         n_tiles = ceil_div(p->ncols, ct);
     }
@@ -79,22 +79,26 @@ int plan_modgemm(vipir_modgemm_plan* p) {
     g.n_chunks = ceil_div(g.atoms, vipir::MG_MAX_CHUNK_ATOMS);
     g.atoms_per_chunk = ceil_div(g.atoms, g.n_chunks);
     g.b_stage_bytes = vipir::MG_BK * ct * (4 / cg);
-    g.b_stages = tune_env("VIPIR_TUNE_MG_BSTAGES", 3);
-    if (g.b_stages < 2) g.b_stages = 2;
+    g.b_stages = p->tune.b_stages ? p->tune.b_stages : 3;
+    // barrier area: 2 x 8 bytes per ring slot, 4 accumulator barriers, the TMEM base word (<= 512 bytes: the
+    // tuning domain caps b_stages at 4 and a_stages at 24)
     const uint32_t overhead = 1024 /* alignment */ + vipir::MG_ZERO_BYTES + 512 /* barriers */;
+    if (overhead + g.b_stages * g.b_stage_bytes + 4 * vipir::MG_A_BYTES > kMaxSmem) return VIPIR_ERR_UNSUPPORTED;
     const uint32_t left = kMaxSmem - overhead - g.b_stages * g.b_stage_bytes;
     g.a_stages = left / vipir::MG_A_BYTES;
-    const uint32_t a_force = tune_env("VIPIR_TUNE_MG_ASTAGES", 0);
-    if (a_force >= 2 && a_force < g.a_stages) g.a_stages = a_force;
-    if (g.a_stages < 4) return VIPIR_ERR_UNSUPPORTED;
     if (g.a_stages > 24) g.a_stages = 24;
+    if (const uint32_t a_force = p->tune.a_stages) {
+        if (a_force > g.a_stages) return VIPIR_ERR_UNSUPPORTED;
+        g.a_stages = a_force;
+    }
+    if (g.a_stages < 4) return VIPIR_ERR_UNSUPPORTED;
+    static_assert(16 * 24 + 16 * 4 + 36 <= 512, "barrier area");
     g.acc_stages = (2 * 7 * ct <= 512) ? 2u : 1u;
     uint32_t tc = 32;
     while (tc < g.acc_stages * 7 * ct) tc <<= 1;
     g.tmem_cols = tc;
     g.idesc = (2u << 4) /* D = s32 */ | (0u << 7) /* A = u8 */ | (0u << 10) /* B = u8 */ | (((4 * ct) >> 3) << 17) |
               (((128u * cg) >> 4) << 24);
-    g.dbg = tune_env("VIPIR_TUNE_MG_DBG", 0);
     for (uint32_t t = 0; t < p->T; ++t) {
         const uint32_t q = p->moduli[t];
         g.moduli[t] = q;
@@ -164,8 +168,21 @@ extern "C" {
 
 int vipir_modgemm_plan_create(vipir_modgemm_plan** out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K, uint32_t ncols,
                               uint32_t gcols, const uint32_t* moduli) {
+    return vipir_modgemm_plan_create_tuned(out, T, NC, M, K, ncols, gcols, moduli, nullptr);
+}
+
+int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64_t NC, uint32_t M, uint32_t K,
+                                    uint32_t ncols, uint32_t gcols, const uint32_t* moduli,
+                                    const vipir_modgemm_tuning* tune) {
     if (!out) return VIPIR_ERR_INVALID_ARG;
     *out = nullptr;
+    if (tune) {
+        if (tune->cta_group > 2 || tune->tile_cols > 64 || tune->tile_cols % 8 != 0 || tune->b_stages == 1 ||
+            tune->b_stages > 4 || (tune->a_stages != 0 && tune->a_stages < 4) || tune->a_stages > 24)
+            return VIPIR_ERR_INVALID_ARG;
+        for (uint32_t r : tune->reserved)
+            if (r != 0) return VIPIR_ERR_INVALID_ARG;
+    }
     if (!moduli || T == 0 || T > VIPIR_MAX_MODULI || NC == 0 || M == 0 || K == 0 || ncols == 0 || gcols > ncols)
         return VIPIR_ERR_INVALID_ARG;
     for (uint32_t t = 0; t < T; ++t)
@@ -193,11 +210,11 @@ int vipir_modgemm_plan_create(vipir_modgemm_plan** out, uint32_t T, uint64_t NC,
     p->gcols = gcols;
     p->num_sms = sms;
     for (uint32_t t = 0; t < T; ++t) p->moduli[t] = moduli[t];
+    if (tune) p->tune = *tune;
     // CTA pairs (one 256-row tile, each CTA staging half of the C limb tile) once the C tile is wide
-    // enough for its shared-memory traffic to matter; VIPIR_TUNE_MG_CG overrides
+    // enough for its shared-memory traffic to matter
     p->cg = (M > 128 && ncols >= 16) ? 2u : 1u;  // measured: pairs win from 16 columns up (8 clients: 2.64 -> 2.55 ms)
-    const uint32_t cg_force = tune_env("VIPIR_TUNE_MG_CG", 0);
-    if (cg_force == 1 || cg_force == 2) p->cg = cg_force;
+    if (p->tune.cta_group) p->cg = p->tune.cta_group;
     p->hp_bytes = p->P * M * 4ull * p->Kp;
     p->cp_bytes = p->P * 4ull * ncols * p->Kp;
     if (cudaMalloc(&p->d_hp, p->hp_bytes) != cudaSuccess || cudaMalloc(&p->d_cp, p->cp_bytes) != cudaSuccess) {
@@ -262,8 +279,13 @@ int vipir_modgemm_info(const vipir_modgemm_plan* p, vipir_modgemm_info_t* o) {
     o->launches = 2;
     o->h_limb_bytes = p->hp_bytes;
     o->c_limb_bytes = p->cp_bytes;
-    o->d_h_limbs = p->d_hp;
-    o->d_c_limbs = p->d_cp;
+    return VIPIR_OK;
+}
+
+int vipir_testing_modgemm_limbs(const vipir_modgemm_plan* p, void** d_h_limbs, void** d_c_limbs) {
+    if (!p || !d_h_limbs || !d_c_limbs) return VIPIR_ERR_INVALID_ARG;
+    *d_h_limbs = p->d_hp;
+    *d_c_limbs = p->d_cp;
     return VIPIR_OK;
 }
 

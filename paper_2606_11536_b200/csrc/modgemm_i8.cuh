@@ -61,7 +61,6 @@ struct ModGemmParams {
     uint32_t a_stages, b_stages, b_stage_bytes;  // per CTA
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
-    uint32_t dbg;      // timing experiments only (VIPIR_TUNE_MG_DBG): bit0 no D offset, bit1 no epilogue math
     uint32_t moduli[MG_MAX_MODULI];
     uint32_t w[MG_MAX_MODULI][3];     // 2^32, 2^40, 2^48 mod q_t: weights of the three high limb sums
     uint64_t barrett[MG_MAX_MODULI];  // floor(2^64 / q_t)
@@ -265,7 +264,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
                             for (uint32_t kk = 0; kk < MG_BK / MG_UMMA_K; ++kk) {
                                 const uint64_t koff = (uint64_t)((kk * MG_UMMA_K) >> 4);
-                                ptx::mma_i8<CG>(tacc + ((p.dbg & 1) ? 0u : i * p.ct), dA + koff, dB + koff, p.idesc,
+                                ptx::mma_i8<CG>(tacc + i * p.ct, dA + koff, dB + koff, p.idesc,
                                                 (first && kk == 0) ? 0u : 1u);
                             }
                             if constexpr (CG == 2) ptx::tc_commit_pair(&emptyA[sa], 3);
@@ -293,7 +292,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         const uint32_t quarter = warp & 3;
         const uint32_t half = (warp - 4) >> 2;
         const uint32_t g0 = p.ncols - p.gcols;
-        const uint32_t n_groups = (p.dbg & 2) ? 0u : p.ct / 8;  // <= 8
+        const uint32_t n_groups = p.ct / 8;  // <= 8
         uint32_t acc_it = 0;
         for (uint32_t u = unit0; u < n_units; u += unit_stride) {
             const uint32_t prob = u / tiles_per_problem, rem = u % tiles_per_problem;

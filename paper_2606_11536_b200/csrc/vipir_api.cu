@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/vipir.h"
+#include "../../include/vipir_testing.h"
 #include "db_split.cuh"
 #include "gemm_i8_tcgen05.cuh"
 #include "gemv_b1.cuh"
@@ -29,7 +30,6 @@ int cuda_fail(cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail(e__, #call);      \
     } while (0)
 
-uint32_t tune_env(const char* name, uint32_t dflt);
 // the opt-in shared-memory attribute of a kernel is per device: true the first time the calling thread
 // asks on the current device
 bool attr_needed(uint64_t& done_mask) {
@@ -82,11 +82,6 @@ int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint3
     return VIPIR_OK;
 }
 
-// tuning override read at plan time (experiments only; unset = the planner's own choice)
-uint32_t tune_env(const char* name, uint32_t dflt) {
-    const char* v = getenv(name);
-    return (v && *v) ? (uint32_t)strtoul(v, nullptr, 10) : dflt;
-}
 uint32_t round_up(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
 uint32_t ceil_div(uint32_t x, uint32_t m) { return (x + m - 1) / m; }
 
@@ -101,6 +96,7 @@ struct vipir_plan {
     uint32_t regime;
     uint32_t ms_bits;  // fused modulus switch (0 = off)
     uint32_t db_signed;  // DB elements are two's-complement int8
+    vipir_tuning tune;   // explicit planner overrides (vipir_dbmul_plan_tuned); all zero = the planner's own choices
     int num_sms;
     // workspace
     uint8_t* d_planes;
@@ -175,6 +171,7 @@ int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaSt
 int plan_gemm(vipir_plan* p, int cg) {
     vipir::GemmParams& g = p->gm;
     memset(&g, 0, sizeof g);
+    if (p->tune.separate_split) return VIPIR_ERR_UNSUPPORTED;  // the tensor-core regimes always run the splitter
     const uint32_t lc = p->lc;
     // limb-plane u16 DB: the two limb tiles of a row block are two M sub-tiles, so msub >= 2
     const uint32_t nl = (p->db_layout == VIPIR_DB_LIMB_PLANES) ? 2u : 1u;
@@ -188,8 +185,10 @@ int plan_gemm(vipir_plan* p, int cg) {
         n_tiles = ceil_div(p->nq, qt_max);
         qt = round_up(ceil_div(p->nq, n_tiles), q_align);
     }
-    const uint32_t qt_force = tune_env("VIPIR_TUNE_QT", 0);
-    if (qt_force >= q_align && qt_force % q_align == 0 && qt_force <= qt_max) qt = qt_force;
+    if (const uint32_t qt_force = p->tune.tile_queries) {
+        if (qt_force % q_align != 0 || qt_force > qt_max) return VIPIR_ERR_UNSUPPORTED;
+        qt = qt_force;
+    }
     uint32_t bn = qt * lc;
     if (bn > 256) {
         qt = round_up(qt, q_align2);
@@ -207,10 +206,10 @@ int plan_gemm(vipir_plan* p, int cg) {
     g.total_ksteps = (uint32_t)((p->kbytes + vipir::GM_BK - 1) / vipir::GM_BK);
     const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;  // 256
     g.n_chunks = ceil_div(g.total_ksteps, max_ksteps);
-    {
-        // experiments: finer work items for short K (profiles/r01_tuning.md section 6: no robust gain, not a rule)
-        const uint32_t min_chunks = tune_env("VIPIR_TUNE_MIN_CHUNKS", 0);
-        if (min_chunks > g.n_chunks && min_chunks <= g.total_ksteps) g.n_chunks = min_chunks;
+    if (const uint32_t min_chunks = p->tune.min_chunks) {
+        // finer work items for short K (measured: no robust gain, so not a planner rule)
+        if (min_chunks > g.total_ksteps) return VIPIR_ERR_UNSUPPORTED;
+        if (min_chunks > g.n_chunks) g.n_chunks = min_chunks;
     }
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
     const uint32_t max_groups = (uint32_t)p->num_sms / cg;
@@ -228,20 +227,21 @@ int plan_gemm(vipir_plan* p, int cg) {
             break;
         }
     }
-    const uint32_t msub_force = tune_env("VIPIR_TUNE_MSUB", 0);
-    if ((msub_force == 1 || msub_force == 2 || msub_force == 4) && msub_force * bn <= 512 && msub_force % nl == 0)
+    if (const uint32_t msub_force = p->tune.m_sub) {
+        if (msub_force * bn > 512 || msub_force % nl != 0) return VIPIR_ERR_UNSUPPORTED;
         msub = msub_force;
+    }
     g.msub = msub;
     const uint64_t rows_unit = 128ull * cg * (msub / nl);
     g.m_tiles = (uint32_t)((p->rows + rows_unit - 1) / rows_unit);
     g.atom_bytes = msub * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
     const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
-    // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes"); VIPIR_TUNE_* override
+    // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes")
     // measured on B200 (profiles/r01_tuning.md): several k-atoms per stage (longer contiguous DB
     // runs per row, fewer barrier round trips) beat deeper rings of single atoms; keep >= 3 stages
     uint32_t katoms = (kMaxSmem - overhead) / 3 / g.atom_bytes;
     if (katoms > 4) katoms = 4;
-    katoms = tune_env("VIPIR_TUNE_KATOMS", katoms);
+    if (p->tune.k_atoms) katoms = p->tune.k_atoms;
     if (katoms < 1) katoms = 1;
     while (katoms > 1 && 2 * katoms * g.atom_bytes > kMaxSmem - overhead) --katoms;
     if (katoms > g.ksteps_per_chunk) katoms = g.ksteps_per_chunk;
@@ -249,8 +249,10 @@ int plan_gemm(vipir_plan* p, int cg) {
     g.stage_bytes = katoms * g.atom_bytes;
     uint32_t stages = (kMaxSmem - overhead) / g.stage_bytes;
     if (stages > 12) stages = 12;
-    const uint32_t want = tune_env("VIPIR_TUNE_GEMM_STAGES", 0);
-    if (want >= 2 && want < stages) stages = want;
+    if (const uint32_t want = p->tune.stages) {
+        if (want > stages) return VIPIR_ERR_UNSUPPORTED;
+        stages = want;
+    }
     if (stages < 2) return VIPIR_ERR_UNSUPPORTED;
     g.stages = stages;
     g.acc_stages = (2 * msub * bn <= 512) ? 2u : 1u;
@@ -267,8 +269,8 @@ int plan_gemm(vipir_plan* p, int cg) {
     p->smem_bytes = stages * g.stage_bytes + overhead;
     // groups: one per SM (pair); fewer only when there are fewer work items (unit, K chunk) than that
     const uint64_t items = (uint64_t)g.m_tiles * g.n_tiles * g.n_chunks;
-    g.split = tune_env("VIPIR_TUNE_SPLIT", 1);
-    g.collector = tune_env("VIPIR_TUNE_COLLECTOR", 1);
+    g.split = p->tune.whole_units ? 0u : 1u;
+    g.collector = p->tune.no_collector ? 0u : 1u;
     const uint64_t n_units64 = (uint64_t)g.m_tiles * g.n_tiles;
     g.n_groups = (uint32_t)(items < max_groups ? items : max_groups);
     if (!g.split && n_units64 < g.n_groups) g.n_groups = (uint32_t)n_units64;
@@ -289,18 +291,20 @@ int plan_gemm(vipir_plan* p, int cg) {
 
 int plan_gemv(vipir_plan* p) {
     if (p->nq != 1 || p->n_moduli != 0 || p->lc != 4) return VIPIR_ERR_UNSUPPORTED;
+    const vipir_tuning& tu = p->tune;  // overrides of the tensor-core regimes do not apply here
+    if (tu.m_sub || tu.tile_queries || tu.k_atoms || tu.min_chunks || tu.whole_units || tu.no_collector)
+        return VIPIR_ERR_UNSUPPORTED;
     vipir::GemvParams& g = p->gv;
     memset(&g, 0, sizeof g);
     g.rows = p->rows;
     g.kbytes = (uint32_t)p->kbytes;
     g.n_ksteps = (uint32_t)((p->kbytes + vipir::GV_KT - 1) / vipir::GV_KT);
     g.n_blocks = (uint32_t)((p->rows + vipir::GV_R - 1) / vipir::GV_R);
-    g.stages = tune_env("VIPIR_TUNE_GEMV_STAGES", 4);  // 4 x 36 KiB in flight per SM measured best
-    if (g.stages < 2) g.stages = 2;
-    if (g.stages > 6) g.stages = 6;
+    g.stages = p->tune.stages ? p->tune.stages : 4;  // 4 x 36 KiB in flight per SM measured best
+    if (g.stages > 6) return VIPIR_ERR_UNSUPPORTED;
     p->smem_bytes = g.stages * vipir::GV_STAGE_BYTES + 1024 + 2 * 8 * g.stages + 2 * vipir::GV_R * 4;
     // step a1 fused into the scan when the raw query can be boxed as 32-word rows (gemv_b1.cuh "FUSED")
-    p->gv_fused = p->dl == 1 && p->cols % 32 == 0 && tune_env("VIPIR_TUNE_GEMV_FUSED", 1) != 0;
+    p->gv_fused = p->dl == 1 && p->cols % 32 == 0 && !p->tune.separate_split;
     p->grid = g.n_blocks < (uint32_t)p->num_sms ? g.n_blocks : (uint32_t)p->num_sms;
     // limb planes [4][K'] viewed as u32 elements: box 256 elements (1024 B) x 4 rows
     return make_tmap_2d(&p->tm_planes, p->d_planes, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, p->kbytes / 4, 4, p->kbytes,
@@ -317,8 +321,7 @@ int encode_db_map(vipir_plan* p, const void* d_db) {
         // limb planes: D_hi lies directly behind D_lo, one u8 matrix of 2*rows rows
         rc = make_tmap_2d(&p->tm_db, d_db, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, p->kbytes,
                           p->rows * (p->db_layout == VIPIR_DB_LIMB_PLANES ? 2 : 1), p->kbytes,
-                          vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B,
-                          (CUtensorMapL2promotion)tune_env("VIPIR_TUNE_L2PROMO", CU_TENSOR_MAP_L2_PROMOTION_L2_256B));
+                          vipir::GM_BK, vipir::GM_BM, CU_TENSOR_MAP_SWIZZLE_128B);
     if (rc == VIPIR_OK) p->tm_db_for = d_db;
     return rc;
 }
@@ -348,8 +351,22 @@ int vipir_dbmul_plan_ex(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t
 
 int vipir_dbmul_plan_layout(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
                             const vipir_modulus_spec* mod, uint32_t regime, uint32_t db_layout) {
+    return vipir_dbmul_plan_tuned(out, rows, cols, batch, db_bits, mod, regime, db_layout, nullptr);
+}
+
+int vipir_dbmul_plan_tuned(vipir_plan** out, uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                           const vipir_modulus_spec* mod, uint32_t regime, uint32_t db_layout,
+                           const vipir_tuning* tune) {
     if (!out) return VIPIR_ERR_INVALID_ARG;
     *out = nullptr;
+    if (tune) {  // domain of every field; whether the shape can honour it is the planner's UNSUPPORTED
+        if ((tune->m_sub != 0 && tune->m_sub != 1 && tune->m_sub != 2 && tune->m_sub != 4) || tune->tile_queries > 128 ||
+            tune->k_atoms > 8 || tune->stages == 1 || tune->stages > 12 || tune->separate_split > 1 ||
+            tune->whole_units > 1 || tune->no_collector > 1 || tune->host_staged > 1)
+            return VIPIR_ERR_INVALID_ARG;
+        for (uint32_t r : tune->reserved)
+            if (r != 0) return VIPIR_ERR_INVALID_ARG;
+    }
     // ---- argument checks first: these need no device ----
     if (rows == 0 || cols == 0 || batch == 0) return VIPIR_ERR_INVALID_ARG;
     if (db_bits != 8 && db_bits != 16) return VIPIR_ERR_INVALID_ARG;
@@ -398,6 +415,7 @@ int vipir_dbmul_plan_layout(vipir_plan** out, uint64_t rows, uint64_t cols, uint
     p->nq = T * batch;
     p->lc = (kdl == 2 && n_moduli > 0) ? 5u : 4u;  // split_limbs.cuh: the s = 4 column vanishes mod 2^32
     p->num_sms = sms;
+    if (tune) p->tune = *tune;
 
     if (regime == VIPIR_REGIME_AUTO) {
         if (p->nq == 1 && n_moduli == 0 && !planes) regime = VIPIR_REGIME_GEMV;
@@ -535,7 +553,7 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     // batch-1 scan into pinned, device-mapped host memory: the kernel's plain 128-byte answer stores go straight
     // over PCIe while the scan runs, and the device-to-host copy after it disappears.  (The tensor-core regimes
     // read-modify-write the answer between K chunks and keep the staging buffer.)
-    if (p->regime == VIPIR_REGIME_GEMV && tune_env("VIPIR_TUNE_HOST_DIRECT", 1)) {
+    if (p->regime == VIPIR_REGIME_GEMV && !p->tune.host_staged) {
         cudaPointerAttributes attr{};
         if (cudaPointerGetAttributes(&attr, h_answer) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
             attr.devicePointer != nullptr) {
@@ -596,7 +614,6 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     o->smem_bytes = p->smem_bytes;
     o->grid = p->grid;
     o->workspace_bytes = p->planes_bytes;
-    o->d_limb_planes = p->d_planes;
     o->modswitch_bits = p->ms_bits;
     o->db_signed = p->db_signed;
     o->db_layout = p->db_layout;
@@ -620,8 +637,8 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     return VIPIR_OK;
 }
 
-int vipir_debug_work_items(uint32_t g, uint32_t n_groups, uint32_t n_units, uint32_t n_chunks, uint32_t split,
-                           uint32_t* out_triples, uint32_t cap, uint32_t* n) {
+int vipir_testing_work_items(uint32_t g, uint32_t n_groups, uint32_t n_units, uint32_t n_chunks, uint32_t split,
+                             uint32_t* out_triples, uint32_t cap, uint32_t* n) {
     if (!n || n_groups == 0 || g >= n_groups || n_chunks == 0 || (cap && !out_triples)) return VIPIR_ERR_INVALID_ARG;
     const vipir::WorkPlan w = vipir::make_work_plan(g, n_groups, n_units, n_chunks, split);
     uint32_t count = 0;

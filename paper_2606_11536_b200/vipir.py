@@ -24,17 +24,34 @@ MAX_MODULI = 4
 
 # every symbol include/vipir.h declares
 SYMBOLS = (
-    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul_plan_layout", "vipir_db_split_u16", "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
+    "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul_plan_layout", "vipir_dbmul_plan_tuned", "vipir_db_split_u16",
+    "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
     "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
-    "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error", "vipir_debug_work_items",
-    "vipir_modgemm_plan_create", "vipir_modgemm_set_h", "vipir_modgemm", "vipir_modgemm_split_c",
-    "vipir_modgemm_products", "vipir_modgemm_info", "vipir_modgemm_destroy",
+    "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
+    "vipir_modgemm_plan_create", "vipir_modgemm_plan_create_tuned", "vipir_modgemm_set_h", "vipir_modgemm",
+    "vipir_modgemm_split_c", "vipir_modgemm_products", "vipir_modgemm_info", "vipir_modgemm_destroy",
     "vipir_ntt_plan_create", "vipir_ntt_lift", "vipir_ntt_bad_input", "vipir_ntt_destroy",
 )
+# include/vipir_testing.h: introspection for the test suite, not part of the product ABI
+TESTING_SYMBOLS = ("vipir_testing_work_items", "vipir_testing_modgemm_limbs")
 
 
 class ModulusSpec(ctypes.Structure):
     _fields_ = [("count", ctypes.c_uint32), ("moduli", ctypes.POINTER(ctypes.c_uint32))]
+
+
+class Tuning(ctypes.Structure):
+    """vipir_tuning: explicit planner overrides, every field 0 = the planner's own choice."""
+    _fields_ = [("m_sub", ctypes.c_uint32), ("tile_queries", ctypes.c_uint32), ("k_atoms", ctypes.c_uint32),
+                ("stages", ctypes.c_uint32), ("min_chunks", ctypes.c_uint32), ("separate_split", ctypes.c_uint32),
+                ("whole_units", ctypes.c_uint32), ("no_collector", ctypes.c_uint32), ("host_staged", ctypes.c_uint32),
+                ("reserved", ctypes.c_uint32 * 7)]
+
+
+class ModGemmTuning(ctypes.Structure):
+    """vipir_modgemm_tuning."""
+    _fields_ = [("cta_group", ctypes.c_uint32), ("tile_cols", ctypes.c_uint32), ("a_stages", ctypes.c_uint32),
+                ("b_stages", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 4)]
 
 
 class Info(ctypes.Structure):
@@ -44,7 +61,7 @@ class Info(ctypes.Structure):
         ("n_chunks", ctypes.c_uint32), ("tile_queries", ctypes.c_uint32), ("tile_cols", ctypes.c_uint32),
         ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32), ("n_tiles", ctypes.c_uint32),
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
-        ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64), ("d_limb_planes", ctypes.c_void_p),
+        ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64),
         ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32), ("m_sub", ctypes.c_uint32),
         ("db_layout", ctypes.c_uint32),
     ]
@@ -62,7 +79,7 @@ class ModGemmInfo(ctypes.Structure):
         ("n_tiles", ctypes.c_uint32), ("n_chunks", ctypes.c_uint32), ("a_stages", ctypes.c_uint32),
         ("b_stages", ctypes.c_uint32), ("acc_stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
         ("grid", ctypes.c_uint32), ("launches", ctypes.c_uint32), ("h_limb_bytes", ctypes.c_uint64),
-        ("c_limb_bytes", ctypes.c_uint64), ("d_h_limbs", ctypes.c_void_p), ("d_c_limbs", ctypes.c_void_p),
+        ("c_limb_bytes", ctypes.c_uint64),
     ]
 
     def as_dict(self):
@@ -99,6 +116,8 @@ def load() -> ctypes.CDLL:
         lib.vipir_dbmul_plan_ex.argtypes = [pp, u64, u64, u32, u32, ms, u32]
         lib.vipir_dbmul_plan_layout.restype = i
         lib.vipir_dbmul_plan_layout.argtypes = [pp, u64, u64, u32, u32, ms, u32, u32]
+        lib.vipir_dbmul_plan_tuned.restype = i
+        lib.vipir_dbmul_plan_tuned.argtypes = [pp, u64, u64, u32, u32, ms, u32, u32, ctypes.POINTER(Tuning)]
         lib.vipir_db_split_u16.restype = i
         lib.vipir_db_split_u16.argtypes = [vp, vp, u64, u64, vp]
         lib.vipir_dbmul.restype = i
@@ -117,11 +136,16 @@ def load() -> ctypes.CDLL:
         lib.vipir_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.vipir_destroy.restype = None
         lib.vipir_destroy.argtypes = [vp]
-        lib.vipir_debug_work_items.restype = i
-        lib.vipir_debug_work_items.argtypes = [u32, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32), u32,
-                                               ctypes.POINTER(ctypes.c_uint32)]
+        lib.vipir_testing_work_items.restype = i
+        lib.vipir_testing_work_items.argtypes = [u32, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32), u32,
+                                                 ctypes.POINTER(ctypes.c_uint32)]
+        lib.vipir_testing_modgemm_limbs.restype = i
+        lib.vipir_testing_modgemm_limbs.argtypes = [vp, pp, pp]
         lib.vipir_modgemm_plan_create.restype = i
         lib.vipir_modgemm_plan_create.argtypes = [pp, u32, u64, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32)]
+        lib.vipir_modgemm_plan_create_tuned.restype = i
+        lib.vipir_modgemm_plan_create_tuned.argtypes = [pp, u32, u64, u32, u32, u32, u32, ctypes.POINTER(ctypes.c_uint32),
+                                                        ctypes.POINTER(ModGemmTuning)]
         lib.vipir_modgemm_set_h.restype = i
         lib.vipir_modgemm_set_h.argtypes = [vp, vp, vp]
         lib.vipir_modgemm.restype = i
@@ -175,8 +199,9 @@ def _ptr(t):
 
 
 def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, regime: int = REGIME_AUTO,
-               db_layout: int = DB_ROW_MAJOR):
-    """vipir_dbmul_plan[_ex|_layout]; returns the opaque plan handle (a c_void_p)."""
+               db_layout: int = DB_ROW_MAJOR, tuning: dict | None = None):
+    """vipir_dbmul_plan[_ex|_layout|_tuned]; returns the opaque plan handle (a c_void_p).
+    tuning: {field of vipir_tuning: value} -- explicit planner overrides."""
     lib = load()
     handle = ctypes.c_void_p()
     spec_p = None
@@ -184,8 +209,13 @@ def dbmul_plan(rows: int, cols: int, batch: int, db_bits: int = 8, moduli=None, 
         arr = (ctypes.c_uint32 * len(moduli))(*[int(m) for m in moduli])
         spec = ModulusSpec(len(moduli), arr)
         spec_p = ctypes.byref(spec)
-    _check(lib.vipir_dbmul_plan_layout(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime, db_layout),
-           "vipir_dbmul_plan")
+    if tuning:
+        tune = Tuning(**{k: int(v) for k, v in tuning.items()})
+        _check(lib.vipir_dbmul_plan_tuned(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime, db_layout,
+                                          ctypes.byref(tune)), "vipir_dbmul_plan_tuned")
+    else:
+        _check(lib.vipir_dbmul_plan_layout(ctypes.byref(handle), rows, cols, batch, db_bits, spec_p, regime, db_layout),
+               "vipir_dbmul_plan")
     return handle
 
 
@@ -241,8 +271,8 @@ class Plan:
     """Context-manager convenience around dbmul_plan / destroy."""
 
     def __init__(self, rows, cols, batch, db_bits=8, moduli=None, regime=REGIME_AUTO, modswitch_bits=0,
-                 db_signed=False, db_layout=DB_ROW_MAJOR):
-        self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime, db_layout)
+                 db_signed=False, db_layout=DB_ROW_MAJOR, tuning=None):
+        self.handle = dbmul_plan(rows, cols, batch, db_bits, moduli, regime, db_layout, tuning)
         if modswitch_bits:
             plan_set_modswitch(self.handle, modswitch_bits)
         if db_signed:
@@ -273,27 +303,39 @@ class Plan:
             pass
 
 
-def debug_work_items(g: int, n_groups: int, n_units: int, n_chunks: int, split: int = 1):
-    """vipir_debug_work_items: [(unit, chunk, must_wait), ...] for group g (host only)."""
+def testing_work_items(g: int, n_groups: int, n_units: int, n_chunks: int, split: int = 1):
+    """vipir_testing_work_items (include/vipir_testing.h): [(unit, chunk, must_wait), ...] for group g (host only)."""
     cap = n_units * n_chunks + 1
     buf = (ctypes.c_uint32 * (3 * cap))()
     n = ctypes.c_uint32(0)
-    _check(load().vipir_debug_work_items(g, n_groups, n_units, n_chunks, split, buf, cap, ctypes.byref(n)),
-           "vipir_debug_work_items")
+    _check(load().vipir_testing_work_items(g, n_groups, n_units, n_chunks, split, buf, cap, ctypes.byref(n)),
+           "vipir_testing_work_items")
     return [(buf[3 * i], buf[3 * i + 1], bool(buf[3 * i + 2])) for i in range(n.value)]
 
 
 # ---- parallel INT32 modular GEMMs  Out = H*C + (0|G) mod q_t  (include/vipir.h, NEXT-4) ----------
 
-def modgemm_plan_create(T: int, NC: int, M: int, K: int, ncols: int, gcols: int, moduli):
-    """vipir_modgemm_plan_create; returns the opaque plan handle."""
+def modgemm_plan_create(T: int, NC: int, M: int, K: int, ncols: int, gcols: int, moduli, tuning: dict | None = None):
+    """vipir_modgemm_plan_create[_tuned]; returns the opaque plan handle."""
     handle = ctypes.c_void_p()
     arr = (ctypes.c_uint32 * max(len(moduli), 1))(*[int(m) for m in moduli])
     if len(moduli) != T:
         raise ValueError(f"{len(moduli)} moduli for T = {T}")
-    _check(load().vipir_modgemm_plan_create(ctypes.byref(handle), T, NC, M, K, ncols, gcols, arr),
-           "vipir_modgemm_plan_create")
+    if tuning:
+        tune = ModGemmTuning(**{k: int(v) for k, v in tuning.items()})
+        _check(load().vipir_modgemm_plan_create_tuned(ctypes.byref(handle), T, NC, M, K, ncols, gcols, arr,
+                                                      ctypes.byref(tune)), "vipir_modgemm_plan_create_tuned")
+    else:
+        _check(load().vipir_modgemm_plan_create(ctypes.byref(handle), T, NC, M, K, ncols, gcols, arr),
+               "vipir_modgemm_plan_create")
     return handle
+
+
+def testing_modgemm_limbs(plan):
+    """vipir_testing_modgemm_limbs (include/vipir_testing.h): device addresses (d_h_limbs, d_c_limbs)."""
+    h, c = ctypes.c_void_p(), ctypes.c_void_p()
+    _check(load().vipir_testing_modgemm_limbs(plan, ctypes.byref(h), ctypes.byref(c)), "vipir_testing_modgemm_limbs")
+    return h.value, c.value
 
 
 def modgemm_set_h(plan, d_H, stream=None):
@@ -329,8 +371,8 @@ def modgemm_destroy(plan):
 class ModGemmPlan:
     """Context-manager convenience around modgemm_plan_create / modgemm_destroy."""
 
-    def __init__(self, T, NC, M, K, ncols, gcols, moduli):
-        self.handle = modgemm_plan_create(T, NC, M, K, ncols, gcols, moduli)
+    def __init__(self, T, NC, M, K, ncols, gcols, moduli, tuning=None):
+        self.handle = modgemm_plan_create(T, NC, M, K, ncols, gcols, moduli, tuning)
         self.info = modgemm_info(self.handle)
 
     def set_h(self, d_H, stream=None):

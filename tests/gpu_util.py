@@ -11,9 +11,10 @@ def ensure_built():
 
 
 def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.REGIME_AUTO, return_info=False,
-              modswitch_bits=0, db_signed=False, db_layout=vipir.DB_ROW_MAJOR):
+              modswitch_bits=0, db_signed=False, db_layout=vipir.DB_ROW_MAJOR, tuning=None):
     """D_host rows x cols (u8/u16), Q_host [T][B][cols] u32 -> answer [T][B][rows] u32 via libvipir.
-    db_layout = DB_LIMB_PLANES: the u16 DB is first re-laid out on the device by vipir_db_split_u16."""
+    db_layout = DB_LIMB_PLANES: the u16 DB is first re-laid out on the device by vipir_db_split_u16.
+    tuning: explicit planner overrides (vipir_tuning fields)."""
     import torch
     ensure_built()
     D_host = np.ascontiguousarray(D_host)
@@ -28,7 +29,7 @@ def run_dbmul(D_host: np.ndarray, Q_host: np.ndarray, moduli=None, regime=vipir.
         d_planes = torch.full_like(d_db, 0x5A)
         vipir.db_split_u16(d_db, d_planes, rows, cols)
         d_db = d_planes
-    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits, db_signed, db_layout) as plan:
+    with vipir.Plan(rows, cols, batch, db_bits, moduli, regime, modswitch_bits, db_signed, db_layout, tuning) as plan:
         plan(d_db, d_q, d_a)
         torch.cuda.synchronize()
         info = plan.info

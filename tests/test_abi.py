@@ -17,13 +17,49 @@ def lib():
     return vipir.load()
 
 
-def test_header_symbols_are_exported(lib):
-    header = (ROOT / "include" / "vipir.h").read_text()
+def _declared(header_name):
+    header = (ROOT / "include" / header_name).read_text()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)  # declarations only, not comments
-    declared = set(re.findall(r"\b(vipir_[a-z0-9_]+)\s*\(", header))
+    return set(re.findall(r"\b(vipir_[a-z0-9_]+)\s*\(", header))
+
+
+def test_header_symbols_are_exported(lib):
+    assert sorted(f.name for f in (ROOT / "include").glob("*.h")) == ["vipir.h", "vipir_testing.h"]
+    declared = _declared("vipir.h")
     assert declared == set(vipir.SYMBOLS), declared ^ set(vipir.SYMBOLS)
-    for name in declared:
+    testing = _declared("vipir_testing.h")
+    assert testing == set(vipir.TESTING_SYMBOLS), testing ^ set(vipir.TESTING_SYMBOLS)
+    for name in declared | testing:
         assert hasattr(lib, name), name
+
+
+def test_library_never_reads_the_environment():
+    """No getenv in the product: every planner override is an explicit vipir_tuning argument."""
+    for f in (ROOT / "paper_2606_11536_b200" / "csrc").glob("*.cu*"):
+        assert "getenv" not in f.read_text(), f
+
+
+def test_tuning_domain_is_checked_before_any_device_call(lib):
+    def st(**fields):
+        h = ctypes.c_void_p()
+        tune = vipir.Tuning(**fields)
+        return lib.vipir_dbmul_plan_tuned(ctypes.byref(h), 256, 1024, 8, 8, None, 0, 0, ctypes.byref(tune))
+    for bad in (dict(m_sub=3), dict(m_sub=8), dict(tile_queries=129), dict(k_atoms=9), dict(stages=1), dict(stages=13),
+                dict(separate_split=2), dict(whole_units=2), dict(no_collector=2), dict(host_staged=2)):
+        assert st(**bad) == vipir.ERR_INVALID_ARG, bad
+    tune = vipir.Tuning()
+    tune.reserved[3] = 1
+    h = ctypes.c_void_p()
+    assert lib.vipir_dbmul_plan_tuned(ctypes.byref(h), 256, 1024, 8, 8, None, 0, 0, ctypes.byref(tune)) == vipir.ERR_INVALID_ARG
+
+    def mg(**fields):
+        h = ctypes.c_void_p()
+        tune = vipir.ModGemmTuning(**fields)
+        q = (ctypes.c_uint32 * 1)(97)
+        return lib.vipir_modgemm_plan_create_tuned(ctypes.byref(h), 1, 2, 128, 128, 8, 0, q, ctypes.byref(tune))
+    for bad in (dict(cta_group=3), dict(tile_cols=12), dict(tile_cols=72), dict(a_stages=3), dict(a_stages=25),
+                dict(b_stages=1), dict(b_stages=5)):
+        assert mg(**bad) == vipir.ERR_INVALID_ARG, bad
 
 
 def test_status_strings(lib):
@@ -86,6 +122,8 @@ def test_null_out_pointer(lib):
     assert lib.vipir_plan_set_modswitch(None, 18) == vipir.ERR_INVALID_ARG
     assert lib.vipir_plan_set_db_signed(None, 1) == vipir.ERR_INVALID_ARG
     assert lib.vipir_dbmul_plan_layout(None, 16, 16, 1, 16, None, 0, 1) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_dbmul_plan_tuned(None, 16, 16, 1, 8, None, 0, 0, None) == vipir.ERR_INVALID_ARG
+    assert lib.vipir_testing_modgemm_limbs(None, None, None) == vipir.ERR_INVALID_ARG
     assert lib.vipir_db_split_u16(None, None, 16, 16, None) == vipir.ERR_INVALID_ARG
 
 

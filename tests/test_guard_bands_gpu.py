@@ -29,17 +29,17 @@ def check_bands(buf):
 
 @pytest.mark.parametrize("regime", [vipir.REGIME_GEMV, vipir.REGIME_MMA_1SM, vipir.REGIME_MMA_2SM])
 @pytest.mark.parametrize("moduli", [None, PRIMES])
-def test_dbmul_writes_only_its_answer(regime, moduli, monkeypatch):
+def test_dbmul_writes_only_its_answer(regime, moduli):
     import torch
     ensure_built()
     if regime == vipir.REGIME_GEMV and moduli:
         pytest.skip("GEMV is q = 2^32 only")
-    monkeypatch.setenv("VIPIR_TUNE_MSUB", "4")
     rows, cols = 128 * 4 * 2 + 77, 32768 + 2064
     batch = 1 if regime == vipir.REGIME_GEMV else 5
     D, Q = inputs.db_rows(91, rows, cols, 8), inputs.query(91, cols, batch, moduli)
     buf, d_a = guarded((Q.shape[0], batch, rows))
-    with vipir.Plan(rows, cols, batch, 8, moduli, regime) as plan:
+    tuning = None if regime == vipir.REGIME_GEMV else {"m_sub": 4}
+    with vipir.Plan(rows, cols, batch, 8, moduli, regime, tuning=tuning) as plan:
         plan(torch.from_numpy(D).cuda(), torch.from_numpy(Q.view(np.int32)).cuda(), d_a)
         torch.cuda.synchronize()
     check_bands(buf)

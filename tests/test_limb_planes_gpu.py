@@ -78,14 +78,13 @@ def test_limb_planes_match_the_u16_definition(regime, moduli, batch):
 @pytest.mark.parametrize("regime", [M1, M2])
 @pytest.mark.parametrize("msub", [2, 4])
 @pytest.mark.parametrize("moduli,bits", [(None, 0), (None, 18), (PRIMES, 0)])
-def test_limb_planes_subtiles_chunks_and_split_units(regime, msub, moduli, bits, monkeypatch):
+def test_limb_planes_subtiles_chunks_and_split_units(regime, msub, moduli, bits):
     # msub = 4: two row blocks x two limb planes per CTA; K: 3 chunks so that leftover units are dealt
     # out chunk by chunk and accumulated through the answer buffer
-    monkeypatch.setenv("VIPIR_TUNE_MSUB", str(msub))
     rows, cols, batch = 128 * 2 * (msub // 2) * 2 + 128 + 37, 32768 * 2 + 2064, 6
     D = inputs.db_rows(400 + msub, rows, cols, 16)
     Q = inputs.query(400 + msub, cols, batch, moduli)
-    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=bits, db_layout=LP)
+    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=bits, db_layout=LP, tuning={"m_sub": msub})
     assert info["m_sub"] == msub and info["n_chunks"] == 3
     want = oracle.dbmul(D, Q, moduli, nthreads=NT)
     if bits:

@@ -3,7 +3,7 @@ NEXT-4): libvipir's tensor-core path, through the C ABI,
 oracle, bit for bit (integer work: no tolerance).
 
 Shapes span several M tiles, N tiles, k-atoms and K chunks with ragged tails in every
-dimension, both CTA groupings (VIPIR_TUNE_MG_CG), all-maximum words at the int32 accumulation
+dimension, both CTA groupings (vipir_modgemm_tuning.cta_group), all-maximum words at the int32 accumulation
 bound, operand words above the modulus, and the paper's own per-problem shape
 (M = 256, K = n = 1280, ncols = 2B; PAPER.md:222-226).
 """
@@ -31,29 +31,21 @@ def run_modgemm(H, C, G, moduli, cg=0, ct=0, return_info=False, via_parts=False)
     T, NC, M, K = H.shape
     ncols = C.shape[2]
     gcols = 0 if G is None else G.shape[2]
-    for name, val in (("VIPIR_TUNE_MG_CG", cg), ("VIPIR_TUNE_MG_CT", ct)):
-        if val:
-            os.environ[name] = str(val)
+    tuning = {k: v for k, v in (("cta_group", cg), ("tile_cols", ct)) if v}
+    d_H = torch.from_numpy(np.ascontiguousarray(H).view(np.int32)).cuda()
+    d_C = torch.from_numpy(np.ascontiguousarray(C).view(np.int32)).cuda()
+    d_G = None if G is None else torch.from_numpy(np.ascontiguousarray(G).view(np.int32)).cuda()
+    d_O = torch.full((T, NC, ncols, M), -1, dtype=torch.int32, device="cuda")  # poison
+    with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli, tuning=tuning) as plan:
+        plan.set_h(d_H)
+        del d_H  # the plan owns its own re-laid-out copy
+        if via_parts:
+            vipir.modgemm_split_c(plan.handle, d_C)
+            vipir.modgemm_products(plan.handle, d_G, d_O)
         else:
-            os.environ.pop(name, None)
-    try:
-        d_H = torch.from_numpy(np.ascontiguousarray(H).view(np.int32)).cuda()
-        d_C = torch.from_numpy(np.ascontiguousarray(C).view(np.int32)).cuda()
-        d_G = None if G is None else torch.from_numpy(np.ascontiguousarray(G).view(np.int32)).cuda()
-        d_O = torch.full((T, NC, ncols, M), -1, dtype=torch.int32, device="cuda")  # poison
-        with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli) as plan:
-            plan.set_h(d_H)
-            del d_H  # the plan owns its own re-laid-out copy
-            if via_parts:
-                vipir.modgemm_split_c(plan.handle, d_C)
-                vipir.modgemm_products(plan.handle, d_G, d_O)
-            else:
-                plan(d_C, d_G, d_O)
-            torch.cuda.synchronize()
-            info = plan.info
-    finally:
-        os.environ.pop("VIPIR_TUNE_MG_CG", None)
-        os.environ.pop("VIPIR_TUNE_MG_CT", None)
+            plan(d_C, d_G, d_O)
+        torch.cuda.synchronize()
+        info = plan.info
     out = d_O.cpu().numpy().view(np.uint32)
     return (out, info) if return_info else out
 
@@ -159,8 +151,9 @@ def test_modgemm_split_kernels_layout():
         torch.cuda.synchronize()
         Kp = plan.info["k_padded"]
         assert Kp == 256
-        hp = _device_bytes(plan.info["d_h_limbs"], plan.info["h_limb_bytes"])
-        cp = _device_bytes(plan.info["d_c_limbs"], plan.info["c_limb_bytes"])
+        d_hp, d_cp = vipir.testing_modgemm_limbs(plan.handle)
+        hp = _device_bytes(d_hp, plan.info["h_limb_bytes"])
+        cp = _device_bytes(d_cp, plan.info["c_limb_bytes"])
     hp = hp.reshape(NC * M, Kp // 128, 4, 128)
     cp = cp.reshape(NC, 4, ncols, Kp)
     Hb = np.zeros((NC * M, Kp), dtype=np.uint32)

@@ -91,13 +91,13 @@ def test_gemv_u8(rows, cols):
 
 @pytest.mark.parametrize("fused", ["1", "0"])
 @pytest.mark.parametrize("signed,bits", [(False, 0), (True, 0), (False, 18)])
-def test_gemv_fused_and_separate_split_agree_with_the_oracle(fused, signed, bits, monkeypatch):
-    """cols % 32 == 0: the query split runs inside the scan kernel (one launch); VIPIR_TUNE_GEMV_FUSED=0
+def test_gemv_fused_and_separate_split_agree_with_the_oracle(fused, signed, bits):
+    """cols % 32 == 0: the query split runs inside the scan kernel (one launch); vipir_tuning.separate_split
     forces the two-launch path.  Ragged rows, a K tail shorter than a stage, several stages."""
-    monkeypatch.setenv("VIPIR_TUNE_GEMV_FUSED", fused)
     rows, cols = 1000, 1024 * 5 + 32 * 7
     D, Q = make(77, rows, cols, 1)
-    got, info = run_dbmul(D, Q, None, G, return_info=True, modswitch_bits=bits, db_signed=signed)
+    got, info = run_dbmul(D, Q, None, G, return_info=True, modswitch_bits=bits, db_signed=signed,
+                          tuning=None if fused == "1" else {"separate_split": 1})
     assert info["launches"] == (1 if fused == "1" else 2)
     want = oracle.dbmul_signed(D, Q, None) if signed else oracle.dbmul(D, Q, None, nthreads=NT)
     if bits:
@@ -180,13 +180,12 @@ def test_mma_config4_launch_path_compared_in_full(regime, cols):
 @pytest.mark.parametrize("regime", [M1, M2])
 @pytest.mark.parametrize("msub", [2, 4])
 @pytest.mark.parametrize("moduli,bits", [(None, 0), (None, 18), (PRIMES, 0)])
-def test_mma_m_subtiles(regime, msub, moduli, bits, monkeypatch):
+def test_mma_m_subtiles(regime, msub, moduli, bits):
     # rows: several (128 * CG * msub)-row units + a ragged tail that leaves whole sub-tiles empty;
     # K: 3 chunks, so units are split between groups and accumulated through the answer buffer
-    monkeypatch.setenv("VIPIR_TUNE_MSUB", str(msub))
     rows, cols, batch = 128 * 2 * msub * 2 + 128 + 37, 32768 * 2 + 2064, 6
     D, Q = make(300 + msub, rows, cols, batch, 8, moduli)
-    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=bits)
+    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=bits, tuning={"m_sub": msub})
     assert info["m_sub"] == msub and info["n_chunks"] == 3
     want = oracle.dbmul(D, Q, moduli, nthreads=NT)
     if bits:
@@ -195,8 +194,7 @@ def test_mma_m_subtiles(regime, msub, moduli, bits, monkeypatch):
 
 
 @pytest.mark.parametrize("regime", [M1, M2])
-def test_mma_m_subtiles_permutation_probe(regime, monkeypatch):
-    monkeypatch.setenv("VIPIR_TUNE_MSUB", "4")
+def test_mma_m_subtiles_permutation_probe(regime):
     rows, cols, batch = 128 * 2 * 4 * 2, 512, 8
     rng = np.random.default_rng(5)
     perm = rng.integers(0, cols, size=rows)
@@ -204,7 +202,7 @@ def test_mma_m_subtiles_permutation_probe(regime, monkeypatch):
     D[np.arange(rows), perm] = 1
     Q = np.stack([(np.arange(cols, dtype=np.uint64) + 1) * (b + 1) * 0x01010101 % (1 << 32) for b in range(batch)])
     Q = Q.astype(np.uint32).reshape(1, batch, cols)
-    got = run_dbmul(D, Q, None, regime)
+    got = run_dbmul(D, Q, None, regime, tuning={"m_sub": 4})
     for b in range(batch):
         assert np.array_equal(got[0, b], Q[0, b, perm]), f"query {b}"
 
@@ -336,6 +334,32 @@ def test_auto_regime_choice():
     with pytest.raises(vipir.VipirError) as e:
         vipir.Plan(1024, 1024, 2, regime=G)
     assert e.value.status == vipir.ERR_UNSUPPORTED
+
+
+def test_tuning_overrides_are_honoured_or_refused():
+    """vipir_dbmul_plan_tuned: an override the shape or regime cannot honour is UNSUPPORTED, never ignored."""
+    ensure_built()
+
+    def status(regime, batch=8, **tuning):
+        try:
+            vipir.Plan(1024, 2048, batch, 8, None, regime, tuning=tuning).close()
+            return vipir.OK
+        except vipir.VipirError as e:
+            return e.status
+    assert status(M2, batch=256, m_sub=2) == vipir.ERR_UNSUPPORTED    # 2 x 512 accumulator columns > TMEM
+    assert status(M1, tile_queries=6) == vipir.ERR_UNSUPPORTED         # not a multiple of 4
+    assert status(M1, tile_queries=128) == vipir.ERR_UNSUPPORTED       # 512 columns need CTA pairs
+    assert status(M1, min_chunks=17) == vipir.ERR_UNSUPPORTED          # only 16 k-atoms
+    assert status(M1, stages=12, k_atoms=4) == vipir.ERR_UNSUPPORTED   # does not fit in shared memory
+    assert status(M1, separate_split=1) == vipir.ERR_UNSUPPORTED       # a GEMV override
+    assert status(G, batch=1, m_sub=2) == vipir.ERR_UNSUPPORTED        # an MMA override
+    assert status(G, batch=1, stages=7) == vipir.ERR_UNSUPPORTED
+    with vipir.Plan(1024, 2048, 8, 8, None, M1, tuning=dict(m_sub=2, tile_queries=4, k_atoms=2, stages=3, min_chunks=4,
+                                                            whole_units=1, no_collector=1)) as p:
+        i = p.info
+        assert (i["m_sub"], i["tile_queries"], i["stages"], i["n_chunks"], i["n_tiles"]) == (2, 4, 3, 4, 2)
+    with vipir.Plan(1024, 2048, 1, 8, None, G, tuning=dict(stages=6, separate_split=1)) as p:
+        assert p.info["stages"] == 6 and p.info["launches"] == 2
 
 
 def test_auto_matches_oracle_on_config_1():

@@ -1,5 +1,5 @@
 """Host-side checks (no GPU) of the tensor-core regimes' work distribution (csrc/gemm_i8_tcgen05.cuh
-"Work distribution"), through vipir_debug_work_items: every (unit, chunk) item is visited exactly once;
+"Work distribution"), through vipir_testing_work_items: every (unit, chunk) item is visited exactly once;
 within a unit chunks are visited in increasing order group by group; a group waits only for groups with
 a lower id, and only after it has worked through every item another group may be waiting for -- the
 argument for deadlock freedom; and the split removes the wave-quantisation loss."""
@@ -25,7 +25,7 @@ def test_every_item_once_and_in_order(G, n_units, nc, split):
     seen = {}
     per_group = []
     for g in range(G):
-        items = vipir.debug_work_items(g, G, n_units, nc, split)
+        items = vipir.testing_work_items(g, G, n_units, nc, split)
         per_group.append(items)
         for pos, (u, c, w) in enumerate(items):
             assert (u, c) not in seen, (u, c)
@@ -53,7 +53,7 @@ def test_waits_point_down_and_producers_come_first(G, n_units, nc):
     owner = {}
     order = {}
     for g in range(G):
-        for pos, (u, c, w) in enumerate(vipir.debug_work_items(g, G, n_units, nc, 1)):
+        for pos, (u, c, w) in enumerate(vipir.testing_work_items(g, G, n_units, nc, 1)):
             owner[(u, c)] = g
             order[(u, c)] = (pos, w)
     for (u, c), g in owner.items():
@@ -61,7 +61,7 @@ def test_waits_point_down_and_producers_come_first(G, n_units, nc):
         if w:
             assert owner[(u, c - 1)] < g
     # simulate: a group advances through its list; a waiting item needs chunk c-1 of its unit done
-    lists = [vipir.debug_work_items(g, G, n_units, nc, 1) for g in range(G)]
+    lists = [vipir.testing_work_items(g, G, n_units, nc, 1) for g in range(G)]
     ptr = [0] * G
     done = set()
     progress = True
@@ -89,7 +89,7 @@ def test_waits_point_down_and_producers_come_first(G, n_units, nc):
 def test_split_balances_the_last_round():
     # BASELINE.json configs[4]: 256 units of 2 chunks on 74 CTA pairs: 7 chunk-items per group instead of 8
     G, n_units, nc = 74, 256, 2
-    assert max(len(vipir.debug_work_items(g, G, n_units, nc, 1)) for g in range(G)) == 7
-    assert max(len(vipir.debug_work_items(g, G, n_units, nc, 0)) for g in range(G)) == 8
+    assert max(len(vipir.testing_work_items(g, G, n_units, nc, 1)) for g in range(G)) == 7
+    assert max(len(vipir.testing_work_items(g, G, n_units, nc, 0)) for g in range(G)) == 8
     # full rounds are round-robin over units (sibling N tiles run side by side)
-    assert [u for u, c, w in vipir.debug_work_items(5, G, n_units, nc, 1)][:6] == [5, 5, 79, 79, 153, 153]
+    assert [u for u, c, w in vipir.testing_work_items(5, G, n_units, nc, 1)][:6] == [5, 5, 79, 79, 153, 153]
