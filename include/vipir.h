@@ -381,7 +381,8 @@ int vipir_ntt_plan_create(vipir_ntt_plan **out, uint32_t T, uint32_t log2n, cons
 int vipir_ntt_lift(vipir_ntt_plan *plan, const uint32_t *d_X, uint32_t n_a, uint32_t M, uint32_t out_layout,
                    uint32_t *d_O, void *cuda_stream);
 
-/* *seen = 1 if any launch since the last call read a word >= 2^p_bits (synchronises the device). */
+/* *seen = 1 if any launch since the last call read a word >= 2^p_bits.  Blocks: cudaDeviceSynchronize() before
+ * the flag is read and after it is cleared, so launches on any stream (blocking or not) are covered. */
 int vipir_ntt_bad_input(vipir_ntt_plan *plan, uint32_t *seen);
 
 /* Free the plan and its tables.  NULL is a no-op. */

@@ -18,10 +18,10 @@
  * M x ncols x K product (M = ceil(D1/N), K = n, ncols = 2B) of 32-bit residues mod q_t, plus
  * the M x gcols matrix G added to the LAST gcols columns ("(0 | G)", gcols = B: the b-parts
  * of the B clients' ciphertexts, eq. (3)'s trivial encryption (0, Delta*iota(b)); DESIGN.md
- * reading R19).
+ * reading R21).
  *
  * Layout ("tile-major (GEMM-friendly)": every problem's operands contiguous;
- * DESIGN.md reading R20).  All arrays uint32:
+ * DESIGN.md reading R21).  All arrays uint32:
  *   H    [T][NC][M][K]        K contiguous
  *   C    [T][NC][ncols][K]    each column of C contiguous along K
  *   G    [T][NC][gcols][M]    (may be NULL when gcols == 0)

@@ -111,7 +111,7 @@ int vipir_ntt_plan_create(vipir_ntt_plan** out, uint32_t T, uint32_t log2n, cons
         return VIPIR_ERR_ALLOC;
     }
     if (cudaMemcpy(p->d_twiddles, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemset(p->d_bad, 0, 4) != cudaSuccess) {
+        cudaMemset(p->d_bad, 0, 4) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
         snprintf(g_cuda_err, sizeof g_cuda_err, "%s", cudaGetErrorString(cudaGetLastError()));
         vipir_ntt_destroy(p);
         return VIPIR_ERR_CUDA;
@@ -153,8 +153,12 @@ int vipir_ntt_lift(vipir_ntt_plan* p, const uint32_t* d_X, uint32_t n_a, uint32_
 
 int vipir_ntt_bad_input(vipir_ntt_plan* p, uint32_t* seen) {
     if (!p || !seen) return VIPIR_ERR_INVALID_ARG;
+    // the flag is written by kernels on the caller's streams (possibly non-blocking ones, which the legacy
+    // stream does not order against): wait for all of them before reading and clearing it
+    CK(cudaDeviceSynchronize());
     CK(cudaMemcpy(seen, p->d_bad, 4, cudaMemcpyDeviceToHost));
     CK(cudaMemset(p->d_bad, 0, 4));
+    CK(cudaDeviceSynchronize());
     return VIPIR_OK;
 }
 

@@ -282,6 +282,9 @@ int plan_gemm(vipir_plan* p, int cg) {
             return VIPIR_ERR_ALLOC;
         }
         CK(cudaMemset(p->d_sync, 0, sync_bytes));
+        // the first launch may come on a non-blocking stream, which the legacy stream's memset is not ordered
+        // against: the plan call may block, so wait for the zeros here
+        CK(cudaDeviceSynchronize());
     }
     g.sync = p->d_sync;
     // limb-plane tensor map: [nq*LC][K'] bytes, box 128 B x (ni_cols / cg) rows, 128B swizzle
