@@ -156,7 +156,9 @@ typedef struct {
     uint32_t no_collector;   /* MMA: 1 = the second N half re-reads the DB operand from shared memory */
     uint32_t host_staged;    /* vipir_dbmul_host: 1 = always stage the answer in device memory and copy it back
                                 (no direct stores into mapped host memory, no overlapped copies) */
-    uint32_t reserved[7];    /* must be 0 */
+    uint32_t host_slices;    /* vipir_dbmul_host, MMA: K slices of the copy / split / scan pipeline, 1..4 (0: three for
+                                queries of 8 MiB and more, else one) */
+    uint32_t reserved[6];    /* must be 0 */
 } vipir_tuning;
 
 /* vipir_dbmul_plan_layout with explicit planner overrides.  Errors: as vipir_dbmul_plan_layout; INVALID_ARG
@@ -187,12 +189,18 @@ int vipir_dbmul(vipir_plan *plan, const void *d_db, const uint32_t *d_query, uin
 /*
  * End-to-end variant with HOST query and answer buffers (the PIR server's per-request path:
  * queries arrive from clients, answers go back; the static DB stays resident on the GPU,
- * PAPER.md:176).  Copies h_query to the device, runs vipir_dbmul, copies the answer back and
- * waits for the stream.  h_query / h_answer: HOST pointers with the d_query / d_answer
- * layouts (pinned memory makes the copies asynchronous); d_db: DEVICE pointer.  The first
- * call allocates device staging owned by the plan.  When h_answer is pinned, device-mapped host memory
- * (cudaHostAlloc / cudaHostRegister) the batch-1 scan stores the answer into it directly and no
- * device-to-host copy is made; the result is complete when the call returns either way.
+ * PAPER.md:176).  Copies h_query to the device, runs the product, delivers the answer to h_answer and
+ * waits for the stream: the result is complete when the call returns.  h_query / h_answer: HOST
+ * pointers with the d_query / d_answer layouts; d_db: DEVICE pointer.  The first call allocates device
+ * staging, a copy stream and events, all owned by the plan.
+ *   Pinned memory (cudaHostAlloc / cudaHostRegister) makes the copies asynchronous.  When h_answer is
+ * pinned and device-mapped, the kernels store the finished answer words into it directly (plain 128-byte
+ * stores over PCIe while the scan runs) and no device-to-host copy is made.
+ *   Tensor-core regimes: the call is pipelined over K slices (PAPER.md:245-249's K chunks, grouped): the
+ * copy stream brings slice i's columns of every query vector and splits them into limbs while the caller's
+ * stream scans slice i-1; every slice adds to the running sums (device staging), the last one writes the
+ * result.  Same answer, bit for bit, as vipir_dbmul.  vipir_tuning.host_staged = 1 selects the plain form
+ * (one copy in, vipir_dbmul, one copy out).
  */
 int vipir_dbmul_host(vipir_plan *plan, const void *d_db, const uint32_t *h_query, uint32_t *h_answer,
                      void *cuda_stream);

@@ -4,6 +4,7 @@
 
 csrc/libvipir.so            the product: C ABI of include/vipir.h
 inputs/libvipir_inputs.so   device twin of the seeded input generator (tests / bench only)
+ceilings/libvipir_ceilings.so   measured ceilings for bench.py: pure int8 MMA loop, register-only butterflies
 """
 from __future__ import annotations
 
@@ -26,6 +27,10 @@ TARGETS = {
     PKG / "inputs" / "libvipir_inputs.so": {
         "src": [PKG / "inputs" / "generator.cu"],
         "deps": [],
+    },
+    PKG / "ceilings" / "libvipir_ceilings.so": {
+        "src": [PKG / "ceilings" / "ceilings.cu"],
+        "deps": [PKG / "csrc" / "ptx.cuh", PKG / "csrc" / "gemm_i8_tcgen05.cuh", PKG / "csrc" / "ntt_lift.cuh"],
     },
 }
 

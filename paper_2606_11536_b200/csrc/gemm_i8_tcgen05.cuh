@@ -72,7 +72,8 @@ struct GemmParams {
     uint32_t n_tiles, m_tiles;
     uint32_t ni_cols;        // N of one MMA instruction
     uint32_t n_instr;        // instructions per k-step (bn = n_instr * ni_cols)
-    uint32_t total_ksteps;   // ceil(K' / 128): number of 128-byte k-atoms
+    uint32_t k_begin;        // first k-atom of this launch's K range (0 unless the call is cut into K slices)
+    uint32_t total_ksteps;   // k-atoms of this launch's K range (ceil(K' / 128) for the whole product)
     uint32_t ksteps_per_chunk;
     uint32_t n_chunks;
     uint32_t katoms;         // k-atoms per pipeline stage (>= 1): one stage = katoms x (A box + B boxes)
@@ -91,7 +92,10 @@ struct GemmParams {
     uint32_t n_moduli;
     uint32_t moduli[GM_MAX_MODULI];
     uint64_t barrett[GM_MAX_MODULI];  // floor(2^64 / p)
-    uint32_t* answer;
+    uint32_t acc_in;         // 1: `answer` already holds the sum over the K range before k_begin (an earlier launch's)
+    uint32_t* answer;        // [nq][rows]: running sums between K chunks, and the result unless final_out differs
+    uint32_t* final_out;     // where the LAST chunk of this launch writes (== answer, or e.g. mapped host memory:
+                             // plain stores only, the running sum is read from `answer`)
 };
 
 // K-major, 128B-swizzled shared-memory operand descriptor (8-row x 128-byte atoms, 1024 B apart)
@@ -280,7 +284,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     for (uint32_t a = 0; a < na; ++a) {
                         uint8_t* sA = sbase + a * p.atom_bytes;
                         uint8_t* sB = sA + p.msub * GM_A_BYTES;
-                        const int32_t k0 = (int32_t)((ks0 + a) * GM_BK);
+                        const int32_t k0 = (int32_t)((p.k_begin + ks0 + a) * GM_BK);
                         if constexpr (CG == 1) {
                             for (uint32_t j = 0; j < p.msub; ++j)
                                 ptx::tma_load_2d(sA + j * GM_A_BYTES, &tmA, &full[stage], k0, sub_row(j), hintA);
@@ -399,8 +403,14 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             // with the fused modulus switch (q = 2^32 only) the LAST chunk needs the running sum back
             // to round it: same batched prefetch, once per tile
             constexpr uint32_t kPf = 8;
-            const bool ms_final = !PRIME && p.ms_bits != 0 && c + 1 == p.n_chunks;
-            const bool need_old = c > 0 && (PRIME || ms_final);
+            const bool first = c == 0 && !p.acc_in;   // nothing accumulated yet: plain store
+            const bool last = c + 1 == p.n_chunks;
+            // the last chunk writes the result to final_out; when that is not the running-sum buffer (the
+            // host call's mapped answer) it needs the running sum back as well, and stores instead of adding
+            const bool redirect = last && p.final_out != p.answer;
+            const bool ms_final = !PRIME && p.ms_bits != 0 && last;
+            const bool need_old = !first && (PRIME || ms_final || redirect);
+            uint32_t* const obase = last ? p.final_out : p.answer;
             for (uint32_t m = 0; m < rsub; ++m) {
                 const uint64_t row = (uint64_t)((mt * rsub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
                 const bool row_ok = row < p.rows;
@@ -429,7 +439,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         for (int i = 0; i < 4; ++i) {
                             const uint32_t q = nt * p.qt + g * 4 + i;
                             if (q < p.nq && row_ok) {
-                                uint32_t* dst = p.answer + (uint64_t)q * p.rows + row;
+                                uint32_t* dst = obase + (uint64_t)q * p.rows + row;
                                 if constexpr (!PRIME) {
                                     // shifts, wrap mod 2^32 (an s = 4 column would vanish)
                                     uint32_t val =
@@ -437,10 +447,12 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                     if constexpr (NL == 2)  // D = D_lo + 2^8 D_hi; the 2^32 term of w[3] vanishes
                                         val += (w[i * LC] << 8) + (w[i * LC + 1] << 16) + (w[i * LC + 2] << 24);
                                     if (ms_final) {
-                                        if (c > 0) val += old[gg * 4 + i];
+                                        if (!first) val += old[gg * 4 + i];
                                         *dst = modswitch_word(val, p.ms_bits);
-                                    } else if (c == 0) {
+                                    } else if (first) {
                                         *dst = val;
+                                    } else if (redirect) {
+                                        *dst = val + old[gg * 4 + i];
                                     } else {
                                         asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
                                     }
@@ -470,7 +482,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                         for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
                                         val = barrett_u64(x, pm, p.barrett[t]);
                                     }
-                                    if (c > 0) {
+                                    if (!first) {
                                         val += old[gg * 4 + i];
                                         if (val >= pm) val -= pm;
                                     }

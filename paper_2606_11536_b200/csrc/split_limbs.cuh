@@ -42,14 +42,16 @@ __device__ __forceinline__ void byte_transpose4(uint32_t a, uint32_t b, uint32_t
 
 // One thread handles 16 consecutive k of one query vector (4 x 128-bit loads).
 // cols must be a multiple of 16/dl (the ABI's 16-byte row rule); tail threads are guarded.
+// Only the columns [k_lo, k_hi) are split (k_lo a multiple of 16; the whole vector: 0, cols) -- the host
+// entry point splits a query slice by slice along K as its copies arrive.
 template <int DL, int LC>
 __global__ void __launch_bounds__(256) split_limbs_kernel(const uint32_t* __restrict__ Q, uint8_t* __restrict__ P,
-                                                          uint64_t cols, uint32_t nq) {
-    const uint64_t groups_per_q = (cols + 15) / 16;
+                                                          uint64_t cols, uint32_t nq, uint64_t k_lo, uint64_t k_hi) {
+    const uint64_t groups_per_q = (k_hi - k_lo + 15) / 16;
     const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= groups_per_q * nq) return;
     const uint32_t q = (uint32_t)(gid / groups_per_q);
-    const uint64_t k0 = (gid % groups_per_q) * 16;
+    const uint64_t k0 = k_lo + (gid % groups_per_q) * 16;
     const uint32_t* src = Q + (uint64_t)q * cols + k0;
     const uint64_t kp = cols * DL;  // plane pitch in bytes
 

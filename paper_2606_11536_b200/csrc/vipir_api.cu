@@ -42,6 +42,7 @@ bool attr_needed(uint64_t& done_mask) {
 }
 constexpr uint32_t kMaxSmem = 232448;  // 227 KiB opt-in dynamic shared memory per CTA
 constexpr uint32_t kChunkBytes = 32768; // 255*255*32768 < 2^31 (R7)
+constexpr uint32_t kMaxHostSlices = 4;  // K slices of one vipir_dbmul_host call (copy / split / scan pipeline)
 
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -102,9 +103,11 @@ struct vipir_plan {
     uint8_t* d_planes;
     uint64_t planes_bytes;
     uint32_t* d_sync;  // MMA regimes: ticket, finished-groups count, per-leftover-unit arrival counters
-    // host-call staging
+    // host-call staging; the copy stream and events of its overlapped form (vipir_dbmul_host)
     uint32_t* d_q_stage;
     uint32_t* d_a_stage;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_begin, ev_slice[kMaxHostSlices];
     // kernel parameters
     vipir::GemmParams gm;
     vipir::GemvParams gv;
@@ -122,14 +125,14 @@ struct vipir_plan {
 namespace {
 
 template <int CG, int LC, bool PRIME, int NL = 1>
-int launch_gemm(vipir_plan* p, cudaStream_t st) {
+int launch_gemm(vipir_plan* p, const vipir::GemmParams& g, cudaStream_t st) {
     auto kern = vipir::gemm_i8_kernel<CG, LC, PRIME, NL>;
     static thread_local uint64_t attr_set = 0;  // bit d: done on device d
     if (attr_needed(attr_set)) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
     }
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(p->grid);
+    cfg.gridDim = dim3(g.n_groups * CG);
     cfg.blockDim = dim3(vipir::GM_THREADS);
     cfg.dynamicSmemBytes = p->smem_bytes;
     cfg.stream = st;
@@ -140,30 +143,34 @@ int launch_gemm(vipir_plan* p, cudaStream_t st) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_db, p->tm_planes, p->gm));
+    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_db, p->tm_planes, g));
     return VIPIR_OK;
 }
 
 template <int CG>
-int launch_gemm_cg(vipir_plan* p, cudaStream_t st) {
+int launch_gemm_cg(vipir_plan* p, const vipir::GemmParams& g, cudaStream_t st) {
     const bool prime = p->n_moduli > 0;
     if (p->db_layout == VIPIR_DB_LIMB_PLANES)
-        return prime ? launch_gemm<CG, 4, true, 2>(p, st) : launch_gemm<CG, 4, false, 2>(p, st);
-    if (p->lc == 5) return launch_gemm<CG, 5, true>(p, st);
-    return prime ? launch_gemm<CG, 4, true>(p, st) : launch_gemm<CG, 4, false>(p, st);
+        return prime ? launch_gemm<CG, 4, true, 2>(p, g, st) : launch_gemm<CG, 4, false, 2>(p, g, st);
+    if (p->lc == 5) return launch_gemm<CG, 5, true>(p, g, st);
+    return prime ? launch_gemm<CG, 4, true>(p, g, st) : launch_gemm<CG, 4, false>(p, g, st);
 }
 
-int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaStream_t st) {
-    const uint64_t groups = ((p->cols + 15) / 16) * p->nq;
+// splits the columns [k_lo, k_hi) of every query vector (k_lo a multiple of 16)
+int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaStream_t st, uint64_t k_lo, uint64_t k_hi) {
+    const uint64_t groups = ((k_hi - k_lo + 15) / 16) * p->nq;
     const uint32_t blocks = (uint32_t)((groups + 255) / 256);
     if (p->kdl == 1)
-        vipir::split_limbs_kernel<1, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+        vipir::split_limbs_kernel<1, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq, k_lo, k_hi);
     else if (p->lc == 4)
-        vipir::split_limbs_kernel<2, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+        vipir::split_limbs_kernel<2, 4><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq, k_lo, k_hi);
     else
-        vipir::split_limbs_kernel<2, 5><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq);
+        vipir::split_limbs_kernel<2, 5><<<blocks, 256, 0, st>>>(d_query, planes, p->cols, p->nq, k_lo, k_hi);
     CK(cudaGetLastError());
     return VIPIR_OK;
+}
+int launch_split(vipir_plan* p, const uint32_t* d_query, uint8_t* planes, cudaStream_t st) {
+    return launch_split(p, d_query, planes, st, 0, p->cols);
 }
 
 // ---- planning ------------------------------------------------------------------------------
@@ -365,7 +372,7 @@ int vipir_dbmul_plan_tuned(vipir_plan** out, uint64_t rows, uint64_t cols, uint3
     if (tune) {  // domain of every field; whether the shape can honour it is the planner's UNSUPPORTED
         if ((tune->m_sub != 0 && tune->m_sub != 1 && tune->m_sub != 2 && tune->m_sub != 4) || tune->tile_queries > 128 ||
             tune->k_atoms > 8 || tune->stages == 1 || tune->stages > 12 || tune->separate_split > 1 ||
-            tune->whole_units > 1 || tune->no_collector > 1 || tune->host_staged > 1)
+            tune->whole_units > 1 || tune->no_collector > 1 || tune->host_staged > 1 || tune->host_slices > kMaxHostSlices)
             return VIPIR_ERR_INVALID_ARG;
         for (uint32_t r : tune->reserved)
             if (r != 0) return VIPIR_ERR_INVALID_ARG;
@@ -462,9 +469,18 @@ int vipir_split_limbs(vipir_plan* p, const uint32_t* d_query, uint8_t* d_planes_
     return launch_split(p, d_query, d_planes_out ? d_planes_out : p->d_planes, static_cast<cudaStream_t>(cuda_stream));
 }
 
+// The launch's view of the K dimension when a call is cut into K slices (vipir_dbmul_host): k-atoms
+// [k_begin, k_begin + k_atoms) of the product, added to what `answer` holds when acc_in is set, the last
+// chunk written to final_out.  The whole product: {0, all, 0, answer}.
+struct KSlice {
+    uint32_t k_begin, k_atoms, acc_in;
+    uint32_t* final_out;
+    bool is_last;
+};
+
 // d_query_fused != NULL: GEMV with the query split fused in (reads the raw query instead of the limb planes)
 static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaStream_t st,
-                     const uint32_t* d_query_fused = nullptr) {
+                     const uint32_t* d_query_fused = nullptr, const KSlice* slice = nullptr) {
     int rc = encode_db_map(p, d_db);
     if (rc != VIPIR_OK) return rc;
     if (p->regime == VIPIR_REGIME_GEMV) {
@@ -479,8 +495,9 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
             CK(cudaFuncSetAttribute(vipir::gemv_b1_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)kMaxSmem));
         }
-        p->gv.answer = d_answer;
-        p->gv.ms_bits = p->ms_bits;
+        vipir::GemvParams gv = p->gv;  // per-call values go into a copy: the plan's parameters stay as planned
+        gv.answer = d_answer;
+        gv.ms_bits = p->ms_bits;
         if (d_query_fused) {  // raw query words, split inside the kernel
             if (p->tm_query_for != d_query_fused) {
                 rc = make_tmap_2d(&p->tm_query, d_query_fused, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, 32, p->cols / 32, 128, 32,
@@ -489,23 +506,37 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
                 p->tm_query_for = d_query_fused;
             }
             if (p->db_signed)
-                vipir::gemv_b1_kernel<true, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, p->gv);
+                vipir::gemv_b1_kernel<true, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, gv);
             else
-                vipir::gemv_b1_kernel<false, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, p->gv);
+                vipir::gemv_b1_kernel<false, true><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_query, gv);
         } else if (p->db_signed) {
-            vipir::gemv_b1_kernel<true, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+            vipir::gemv_b1_kernel<true, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, gv);
         } else {
-            vipir::gemv_b1_kernel<false, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, p->gv);
+            vipir::gemv_b1_kernel<false, false><<<p->grid, vipir::GV_THREADS, p->smem_bytes, st>>>(p->tm_db, p->tm_planes, gv);
         }
         CK(cudaGetLastError());
         return VIPIR_OK;
     }
-    p->gm.answer = d_answer;
-    p->gm.ms_bits = p->ms_bits;
-    p->gm.db_signed = p->db_signed;
+    vipir::GemmParams g = p->gm;  // per-call values go into a copy: the plan's parameters stay as planned
+    g.answer = d_answer;
+    g.final_out = d_answer;
+    g.ms_bits = p->ms_bits;
+    g.db_signed = p->db_signed;
     // instruction descriptor bits [7,10): A operand format, 0 = u8, 1 = s8 (B stays u8: the limbs)
-    p->gm.idesc = (p->gm.idesc & ~(7u << 7)) | ((p->db_signed ? 1u : 0u) << 7);
-    return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, st) : launch_gemm_cg<1>(p, st);
+    g.idesc = (g.idesc & ~(7u << 7)) | ((p->db_signed ? 1u : 0u) << 7);
+    if (slice) {
+        const uint32_t max_ksteps = kChunkBytes / vipir::GM_BK;
+        g.k_begin = slice->k_begin;
+        g.total_ksteps = slice->k_atoms;
+        g.n_chunks = ceil_div(slice->k_atoms, max_ksteps);
+        g.ksteps_per_chunk = ceil_div(slice->k_atoms, g.n_chunks);
+        g.acc_in = slice->acc_in;
+        g.final_out = slice->final_out;
+        if (!slice->is_last) g.ms_bits = 0;  // the switch rounds the complete sum only
+        const uint64_t items = (uint64_t)g.m_tiles * g.n_tiles * g.n_chunks;
+        if (items < g.n_groups) g.n_groups = (uint32_t)items;
+    }
+    return (p->regime == VIPIR_REGIME_MMA_2SM) ? launch_gemm_cg<2>(p, g, st) : launch_gemm_cg<1>(p, g, st);
 }
 
 int vipir_dbmul_scan(vipir_plan* p, const void* d_db, uint32_t* d_answer, void* cuda_stream) {
@@ -542,34 +573,99 @@ int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32
     return scan_only(p, d_db, d_answer, st);
 }
 
+// device pointer of h if it is pinned, device-mapped host memory; else NULL
+static uint32_t* mapped_device_pointer(uint32_t* h) {
+    cudaPointerAttributes attr{};
+    if (cudaPointerGetAttributes(&attr, h) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer)
+        return static_cast<uint32_t*>(attr.devicePointer);
+    cudaGetLastError();  // not a CUDA-known pointer: pageable memory
+    return nullptr;
+}
+
+// K slices of one host call (tensor-core regimes): boundaries in k-atoms.  The first slice is small so that the
+// scan starts early; the copies of the later, larger slices run behind the scan of the earlier ones.
+static uint32_t host_slices(const vipir_plan* p, size_t qbytes, uint32_t bounds[kMaxHostSlices + 1]) {
+    const uint32_t A = p->gm.total_ksteps;
+    uint32_t S = p->tune.host_slices;
+    if (S == 0) S = (qbytes >= (8u << 20) && A >= 16) ? 3u : 1u;  // small queries: one copy, one launch
+    if (S > A) S = A;
+    bounds[0] = 0;
+    // 1/8, 1/2, 1 (three slices); 1/8, 3/8, 5/8, 1 (four); 1/4, 1 (two)
+    static const uint32_t frac8[kMaxHostSlices + 1][kMaxHostSlices] = {{0}, {8}, {2, 8}, {1, 4, 8}, {1, 3, 5, 8}};
+    for (uint32_t i = 0; i < S; ++i) {
+        uint32_t b = (uint32_t)((uint64_t)A * frac8[S][i] / 8);
+        if (b <= bounds[i]) b = bounds[i] + 1;
+        bounds[i + 1] = b;
+    }
+    bounds[S] = A;
+    return S;
+}
+
 int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, uint32_t* h_answer, void* cuda_stream) {
     if (!p || !d_db || !h_query || !h_answer) return VIPIR_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(d_db) & 15) return VIPIR_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t qbytes = (size_t)p->nq * p->cols * 4, abytes = (size_t)p->nq * p->rows * 4;
-    if (!p->d_q_stage) {
-        if (cudaMalloc(&p->d_q_stage, qbytes) != cudaSuccess || cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
-            cudaGetLastError();
-            return VIPIR_ERR_ALLOC;
-        }
+    if (!p->d_q_stage && cudaMalloc(&p->d_q_stage, qbytes) != cudaSuccess) {
+        cudaGetLastError();
+        return VIPIR_ERR_ALLOC;
     }
-    CK(cudaMemcpyAsync(p->d_q_stage, h_query, qbytes, cudaMemcpyHostToDevice, st));
-    // batch-1 scan into pinned, device-mapped host memory: the kernel's plain 128-byte answer stores go straight
-    // over PCIe while the scan runs, and the device-to-host copy after it disappears.  (The tensor-core regimes
-    // read-modify-write the answer between K chunks and keep the staging buffer.)
-    if (p->regime == VIPIR_REGIME_GEMV && !p->tune.host_staged) {
-        cudaPointerAttributes attr{};
-        if (cudaPointerGetAttributes(&attr, h_answer) == cudaSuccess && attr.type == cudaMemoryTypeHost &&
-            attr.devicePointer != nullptr) {
-            int rc = vipir_dbmul(p, d_db, p->d_q_stage, static_cast<uint32_t*>(attr.devicePointer), cuda_stream);
-            if (rc != VIPIR_OK) return rc;
-            CK(cudaStreamSynchronize(st));
-            return VIPIR_OK;
-        }
-        cudaGetLastError();  // not a CUDA-known pointer: pageable memory, fall through to the staged copy
+    // with pinned, device-mapped host memory the kernels store the answer into it directly: their plain 128-byte
+    // stores go over PCIe while the scan runs, and the device-to-host copy after it disappears
+    uint32_t* d_direct = p->tune.host_staged ? nullptr : mapped_device_pointer(h_answer);
+    const bool mma = p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM;
+
+    if (p->regime == VIPIR_REGIME_GEMV && d_direct) {
+        CK(cudaMemcpyAsync(p->d_q_stage, h_query, qbytes, cudaMemcpyHostToDevice, st));
+        int rc = vipir_dbmul(p, d_db, p->d_q_stage, d_direct, cuda_stream);
+        if (rc != VIPIR_OK) return rc;
+        CK(cudaStreamSynchronize(st));
+        return VIPIR_OK;
     }
-    int rc = vipir_dbmul(p, d_db, p->d_q_stage, p->d_a_stage, cuda_stream);
-    if (rc != VIPIR_OK) return rc;
-    CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
+    uint32_t bounds[kMaxHostSlices + 1];
+    const uint32_t S = (mma && !p->tune.host_staged) ? host_slices(p, qbytes, bounds) : 1u;
+    // the running sums between K chunks / slices are read back by the kernels: they stay in device memory
+    const bool need_stage = !d_direct || S > 1 || p->gm.n_chunks > 1 || !mma;
+    if (need_stage && !p->d_a_stage && cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
+        cudaGetLastError();
+        return VIPIR_ERR_ALLOC;
+    }
+    if (!mma || p->tune.host_staged) {  // one copy in, the device call, one copy out
+        CK(cudaMemcpyAsync(p->d_q_stage, h_query, qbytes, cudaMemcpyHostToDevice, st));
+        int rc = vipir_dbmul(p, d_db, p->d_q_stage, p->d_a_stage, cuda_stream);
+        if (rc != VIPIR_OK) return rc;
+        CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return VIPIR_OK;
+    }
+    // ---- tensor-core regimes: copy / split / scan pipelined over K slices ----
+    // copy stream: H2D of slice i's columns of every query vector (a strided copy), its split;  caller's stream:
+    // the scan of slice i, which adds to the running sums of the slices before it.  The last slice's last chunk
+    // writes the finished words to the host buffer (directly when it is mapped).
+    if (!p->copy_stream) {
+        CK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&p->ev_begin, cudaEventDisableTiming));
+        for (uint32_t i = 0; i < kMaxHostSlices; ++i) CK(cudaEventCreateWithFlags(&p->ev_slice[i], cudaEventDisableTiming));
+    }
+    CK(cudaEventRecord(p->ev_begin, st));  // the staging buffers may still be read by work queued on `st`
+    CK(cudaStreamWaitEvent(p->copy_stream, p->ev_begin, 0));
+    uint32_t* const d_final = d_direct ? d_direct : p->d_a_stage;
+    const size_t pitch = (size_t)p->cols * 4;
+    for (uint32_t i = 0; i < S; ++i) {
+        const uint64_t c_lo = (uint64_t)bounds[i] * vipir::GM_BK / p->kdl;
+        uint64_t c_hi = (uint64_t)bounds[i + 1] * vipir::GM_BK / p->kdl;
+        if (c_hi > p->cols) c_hi = p->cols;
+        CK(cudaMemcpy2DAsync(p->d_q_stage + c_lo, pitch, h_query + c_lo, pitch, (size_t)(c_hi - c_lo) * 4, p->nq,
+                             cudaMemcpyHostToDevice, p->copy_stream));
+        int rc = launch_split(p, p->d_q_stage, p->d_planes, p->copy_stream, c_lo, c_hi);
+        if (rc != VIPIR_OK) return rc;
+        CK(cudaEventRecord(p->ev_slice[i], p->copy_stream));
+        CK(cudaStreamWaitEvent(st, p->ev_slice[i], 0));
+        KSlice sl{bounds[i], bounds[i + 1] - bounds[i], i > 0 ? 1u : 0u, i + 1 == S ? d_final : p->d_a_stage, i + 1 == S};
+        rc = scan_only(p, d_db, p->d_a_stage ? p->d_a_stage : d_final, st, nullptr, &sl);
+        if (rc != VIPIR_OK) return rc;
+    }
+    if (!d_direct) CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return VIPIR_OK;
 }
@@ -663,6 +759,11 @@ void vipir_destroy(vipir_plan* p) {
     if (p->d_sync) cudaFree(p->d_sync);
     if (p->d_q_stage) cudaFree(p->d_q_stage);
     if (p->d_a_stage) cudaFree(p->d_a_stage);
+    if (p->copy_stream) {
+        cudaStreamDestroy(p->copy_stream);
+        cudaEventDestroy(p->ev_begin);
+        for (uint32_t i = 0; i < kMaxHostSlices; ++i) cudaEventDestroy(p->ev_slice[i]);
+    }
     delete p;
 }
 

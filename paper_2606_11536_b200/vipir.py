@@ -45,7 +45,7 @@ class Tuning(ctypes.Structure):
     _fields_ = [("m_sub", ctypes.c_uint32), ("tile_queries", ctypes.c_uint32), ("k_atoms", ctypes.c_uint32),
                 ("stages", ctypes.c_uint32), ("min_chunks", ctypes.c_uint32), ("separate_split", ctypes.c_uint32),
                 ("whole_units", ctypes.c_uint32), ("no_collector", ctypes.c_uint32), ("host_staged", ctypes.c_uint32),
-                ("reserved", ctypes.c_uint32 * 7)]
+                ("host_slices", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 6)]
 
 
 class ModGemmTuning(ctypes.Structure):

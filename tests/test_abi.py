@@ -45,7 +45,7 @@ def test_tuning_domain_is_checked_before_any_device_call(lib):
         tune = vipir.Tuning(**fields)
         return lib.vipir_dbmul_plan_tuned(ctypes.byref(h), 256, 1024, 8, 8, None, 0, 0, ctypes.byref(tune))
     for bad in (dict(m_sub=3), dict(m_sub=8), dict(tile_queries=129), dict(k_atoms=9), dict(stages=1), dict(stages=13),
-                dict(separate_split=2), dict(whole_units=2), dict(no_collector=2), dict(host_staged=2)):
+                dict(separate_split=2), dict(whole_units=2), dict(no_collector=2), dict(host_staged=2), dict(host_slices=5)):
         assert st(**bad) == vipir.ERR_INVALID_ARG, bad
     tune = vipir.Tuning()
     tune.reserved[3] = 1

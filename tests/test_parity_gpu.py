@@ -419,6 +419,56 @@ def test_host_entry_point_batch1_pinned_and_pageable(bits):
         assert_same(pinned[:rows].numpy().view(np.uint32).reshape(1, 1, rows), want)
 
 
+# the host call of the tensor-core regimes: copy / split / scan pipelined over K slices, every slice adding to the
+# running sums of the ones before it, the finished words stored straight into mapped host memory (PAPER.md:245-249's
+# K chunks; :176 for the server's per-request path)
+@pytest.mark.parametrize("name,rows,cols,batch,bits,moduli,regime,tune,ms,signed", [
+    ("M1 3 slices", 300, 2064, 8, 8, None, M1, dict(host_slices=3), 0, False),
+    ("M2 4 slices ragged K", 520, 4112, 40, 8, None, M2, dict(host_slices=4), 0, False),
+    ("M2 two N halves, 2 slices", 300, 1040, 130, 8, None, M2, dict(host_slices=2), 0, False),
+    ("M2 slices of two chunks each", 260, 4 * 32768 + 128, 12, 8, None, M2, dict(host_slices=2), 0, False),
+    ("M1 one slice two chunks", 260, 32768 + 256, 8, 8, None, M1, dict(host_slices=1), 0, False),
+    ("M1 planner default (one slice)", 200, 1040, 8, 8, None, M1, None, 0, False),
+    ("M2 primes 3 slices", 300, 2064, 20, 8, PRIMES, M2, dict(host_slices=3), 0, False),
+    ("M1 u16 primes LC=5 3 slices", 260, 1032, 16, 16, PRIMES, M1, dict(host_slices=3), 0, False),
+    ("M2 u16 2^32 byte view", 260, 1032, 24, 16, None, M2, dict(host_slices=3), 0, False),
+    ("M2 modswitch 3 slices", 300, 2064, 40, 8, None, M2, dict(host_slices=3), 18, False),
+    ("M1 signed primes", 300, 2064, 8, 8, PRIMES, M1, dict(host_slices=4), 0, True),
+    ("M2 more groups than units", 130, 8192, 8, 8, None, M2, dict(host_slices=4, m_sub=1), 0, False),
+    ("M2 staged form", 300, 2064, 40, 8, None, M2, dict(host_staged=1), 0, False),
+])
+def test_host_entry_point_tensor_regimes(name, rows, cols, batch, bits, moduli, regime, tune, ms, signed):
+    import torch
+    ensure_built()
+    D, Q = make(91, rows, cols, batch, bits, moduli)
+    D[0, :] = np.iinfo(D.dtype).max  # an all-max row: every slice's partial sum is large
+    want = oracle.dbmul_signed(D, Q, moduli) if signed else oracle.dbmul(D, Q, moduli, nthreads=NT)
+    if ms:
+        want = oracle.modswitch(want, ms)
+    T = Q.shape[0]
+    d_db = torch.from_numpy(D.view(np.uint8).reshape(rows, -1)).cuda()
+    h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+    with vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, signed, tuning=tune) as plan:
+        pinned = torch.full((T * batch * rows + 5,), -1, dtype=torch.int32).pin_memory()
+        for off in (0, 3):  # into mapped host memory, also at an odd word offset
+            pinned.fill_(-1)
+            h_a = pinned[off:off + T * batch * rows]
+            plan.host(d_db, h_q, h_a)
+            assert_same(h_a.numpy().view(np.uint32).reshape(T, batch, rows), want)
+            assert (pinned[:off] == -1).all() and (pinned[off + T * batch * rows:] == -1).all()
+        pageable = torch.full((T, batch, rows), -1, dtype=torch.int32)
+        plan.host(d_db, h_q, pageable)  # staged copy back
+        assert_same(pageable.numpy().view(np.uint32), want)
+        pinned.fill_(-1)
+        plan.host(d_db, torch.from_numpy(Q.view(np.int32).copy()), pinned[:T * batch * rows])  # pageable query
+        assert_same(pinned[:T * batch * rows].numpy().view(np.uint32).reshape(T, batch, rows), want)
+        # the device entry point of the same plan still gives the same words (no plan state was left behind)
+        d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")
+        plan(d_db, torch.from_numpy(Q.view(np.int32)).cuda(), d_a)
+        torch.cuda.synchronize()
+        assert_same(d_a.cpu().numpy().view(np.uint32), want)
+
+
 def test_misaligned_pointers_are_rejected():
     import torch
     ensure_built()
