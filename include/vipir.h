@@ -291,8 +291,10 @@ typedef struct {
     uint32_t n_chunks;      /* K chunks of <= 8192 (int32 accumulation bound 4*255^2*K < 2^31) */
     uint32_t a_stages, b_stages, acc_stages;
     uint32_t smem_bytes, grid;
-    uint32_t launches;      /* kernels enqueued per vipir_modgemm call */
-    uint64_t h_limb_bytes, c_limb_bytes; /* plan-owned workspaces: H limbs [T*NC*M][4*Kp] u8, C limbs [T*NC][4][ncols][Kp] u8 */
+    uint32_t launches;      /* kernels enqueued per vipir_modgemm call: 1 when the C limb split is fused in */
+    uint32_t fused_split;   /* 1: vipir_modgemm splits C inside the products kernel, no C limb planes */
+    uint64_t h_limb_bytes, c_limb_bytes; /* plan-owned workspaces: H limbs [T*NC*M][4*Kp] u8, C limbs [T*NC][4][ncols][Kp] u8
+                                            (0 for a fused plan until vipir_modgemm_split_c is called) */
 } vipir_modgemm_info_t;
 
 /* Explicit planner overrides for the modular GEMMs; every field 0 = the planner's own choice (see vipir_tuning). */
@@ -301,7 +303,10 @@ typedef struct {
     uint32_t tile_cols;   /* ct: columns of C per N tile, a multiple of 8, <= 64 */
     uint32_t a_stages;    /* ring depth of the H operand: 4..24 (at most what fits) */
     uint32_t b_stages;    /* ring depth of the C operand: 2..4 */
-    uint32_t reserved[4]; /* must be 0 */
+    uint32_t c_split;     /* where vipir_modgemm splits C into limbs: 1 = a splitter kernel of its own (two launches),
+                             2 = inside the products kernel (one launch; UNSUPPORTED unless K % 4 == 0) */
+    uint32_t r_stages;    /* fused form: ring depth of the raw C tiles, 2..4 */
+    uint32_t reserved[2]; /* must be 0 */
 } vipir_modgemm_tuning;
 
 /*
@@ -324,13 +329,18 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan **out, uint32_t T, uint64
  * PAPER.md:222).  Must run before the first vipir_modgemm / vipir_modgemm_products. */
 int vipir_modgemm_set_h(vipir_modgemm_plan *plan, const uint32_t *d_H, void *cuda_stream);
 
-/* ONLINE step: enqueue Out = H*C + (0|G) mod q_t: the C limb splitter followed by the tensor-core
- * kernel.  Errors: INVALID_ARG (null / misaligned pointer, set_h not called), CUDA. */
+/* ONLINE step: enqueue Out = H*C + (0|G) mod q_t.  From 32 columns up (and K % 4 == 0: the paper's n = 1280) ONE
+ * kernel: the tensor-core kernel reads the raw words of C by TMA and splits them into limbs in shared memory (the
+ * paper fuses its prmt decomposition into the GEMM kernel as well); below that, where it measures
+ * faster, the C limb splitter followed by the tensor-core kernel (vipir_modgemm_info_t.launches says which;
+ * vipir_modgemm_tuning.c_split overrides).
+ * Errors: INVALID_ARG (null / misaligned pointer, set_h not called), ALLOC, CUDA. */
 int vipir_modgemm(vipir_modgemm_plan *plan, const uint32_t *d_C, const uint32_t *d_G, uint32_t *d_Out,
                   void *cuda_stream);
 
-/* The two kernels of vipir_modgemm separately (per-kernel timing, tests):
- * vipir_modgemm == vipir_modgemm_split_c + vipir_modgemm_products. */
+/* The two-kernel form separately (per-kernel timing, tests; the form a producer that writes C's limb planes
+ * itself would use): vipir_modgemm_split_c writes the plan's C limb planes (allocated on first use),
+ * vipir_modgemm_products multiplies against them.  Same result as vipir_modgemm, bit for bit. */
 int vipir_modgemm_split_c(vipir_modgemm_plan *plan, const uint32_t *d_C, void *cuda_stream);
 int vipir_modgemm_products(vipir_modgemm_plan *plan, const uint32_t *d_G, uint32_t *d_Out, void *cuda_stream);
 

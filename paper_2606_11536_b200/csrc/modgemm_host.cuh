@@ -15,15 +15,18 @@ struct vipir_modgemm_plan {
     uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
     uint64_t hp_bytes, cp_bytes;
     bool h_set;
-    vipir::ModGemmParams mg;
-    uint32_t smem_bytes, grid;
+    bool fused;          // vipir_modgemm splits C inside the products kernel (K % 4 == 0): one launch, no C limb planes
+    vipir::ModGemmParams mg, mg_fused;
+    uint32_t smem_bytes, smem_bytes_fused, grid;
     CUtensorMap tm_h, tm_c;
+    CUtensorMap tm_c_raw;      // FUSED: the caller's raw C words [P][ncols][K] u32
+    const void* tm_c_raw_for;  // d_C the cached tm_c_raw was encoded for
 };
 
 namespace {
 
 int make_tmap_nd(CUtensorMap* m, const void* base, uint32_t rank, const uint64_t* dims, const uint64_t* strides_bytes,
-                 const uint32_t* box) {
+                 const uint32_t* box, CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_UINT8) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) {
         snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled entry point not found");
@@ -37,7 +40,7 @@ int make_tmap_nd(CUtensorMap* m, const void* base, uint32_t rank, const uint64_t
         e[i] = 1;
         if (i + 1 < rank) s[i] = strides_bytes[i];
     }
-    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, rank, const_cast<void*>(base), d, s, b, e,
+    CUresult r = fn(m, dt, rank, const_cast<void*>(base), d, s, b, e,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -80,9 +83,9 @@ int plan_modgemm(vipir_modgemm_plan* p) {
     g.atoms_per_chunk = ceil_div(g.atoms, g.n_chunks);
     g.b_stage_bytes = vipir::MG_BK * ct * (4 / cg);
     g.b_stages = p->tune.b_stages ? p->tune.b_stages : 3;
-    // barrier area: 2 x 8 bytes per ring slot, 4 accumulator barriers, the TMEM base word (<= 512 bytes: the
-    // tuning domain caps b_stages at 4 and a_stages at 24)
-    const uint32_t overhead = 1024 /* alignment */ + vipir::MG_ZERO_BYTES + 512 /* barriers */;
+    // barrier area: 2 x 8 bytes per ring slot, 4 accumulator barriers, the TMEM base word (<= 640 bytes: the
+    // tuning domain caps b_stages at 4 and a_stages at 24; the raw ring has at most 4 slots)
+    const uint32_t overhead = 1024 /* alignment */ + vipir::MG_ZERO_BYTES + 640 /* barriers */;
     if (overhead + g.b_stages * g.b_stage_bytes + 4 * vipir::MG_A_BYTES > kMaxSmem) return VIPIR_ERR_UNSUPPORTED;
     const uint32_t left = kMaxSmem - overhead - g.b_stages * g.b_stage_bytes;
     g.a_stages = left / vipir::MG_A_BYTES;
@@ -92,7 +95,7 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         g.a_stages = a_force;
     }
     if (g.a_stages < 4) return VIPIR_ERR_UNSUPPORTED;
-    static_assert(16 * 24 + 16 * 4 + 36 <= 512, "barrier area");
+    static_assert(16 * 24 + 16 * 4 + 16 * 4 + 36 <= 640, "barrier area");
     g.acc_stages = (2 * 7 * ct <= 512) ? 2u : 1u;
     uint32_t tc = 32;
     while (tc < g.acc_stages * 7 * ct) tc <<= 1;
@@ -106,6 +109,32 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / q);
     }
     p->smem_bytes = g.a_stages * vipir::MG_A_BYTES + g.b_stages * g.b_stage_bytes + overhead;
+    // the fused kernel: two operand slots, two raw-tile slots (ct columns x 128 words each), the rest to the H ring
+    p->mg_fused = g;
+    if (p->fused) {
+        vipir::ModGemmParams& f = p->mg_fused;
+        f.b_stages = p->tune.b_stages ? p->tune.b_stages : 2;
+        // every CTA brings the raw words of the whole tile, per k-atom four 32-word boxes of ct rows (a multiple of
+        // 1 KiB, so every box starts on a swizzle atom).  The raw words of k-atom a are requested when the slot of
+        // atom a - r_stages has been converted; measured at B = 32 (ct = 64, 32 KiB a slot), what the ring takes from
+        // the H ring costs more than a third slot gains (two slots + 8 H boxes 4.95 ms, three + 6: 5.20 ms), so:
+        // the deepest ring that leaves the H ring eight boxes (two k-atoms), at least two slots
+        f.r_stage_bytes = 4 * ct * 128;
+        auto fits = [&](uint32_t r, uint32_t a) {
+            return overhead + f.b_stages * f.b_stage_bytes + r * f.r_stage_bytes + a * vipir::MG_A_BYTES <= kMaxSmem;
+        };
+        f.r_stages = fits(4, 8) ? 4u : fits(3, 8) ? 3u : 2u;
+        if (const uint32_t r_force = p->tune.r_stages) f.r_stages = r_force;
+        const uint32_t fixed = overhead + f.b_stages * f.b_stage_bytes + f.r_stages * f.r_stage_bytes;
+        if (fixed + 4 * vipir::MG_A_BYTES > kMaxSmem) return VIPIR_ERR_UNSUPPORTED;
+        f.a_stages = (kMaxSmem - fixed) / vipir::MG_A_BYTES;
+        if (f.a_stages > 24) f.a_stages = 24;
+        if (const uint32_t a_force = p->tune.a_stages) {
+            if (a_force > f.a_stages) return VIPIR_ERR_UNSUPPORTED;
+            f.a_stages = a_force;
+        }
+        p->smem_bytes_fused = f.a_stages * vipir::MG_A_BYTES + fixed;
+    }
     const uint64_t units = (uint64_t)p->P * g.m_tiles * g.n_tiles;
     if (units >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
     const uint32_t max_units = (uint32_t)p->num_sms / cg;
@@ -119,18 +148,25 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         int rc = make_tmap_nd(&p->tm_h, p->d_hp, 3, dims, str, box);
         if (rc != VIPIR_OK) return rc;
     }
-    // C limb planes [P][4][ncols][Kp]; box = 128 B x ct columns x (4/cg) planes of one problem
-    {
-        const uint64_t dims[4] = {p->Kp, p->ncols, 4, p->P};
-        const uint64_t str[3] = {p->Kp, (uint64_t)p->Kp * p->ncols, 4ull * p->Kp * p->ncols};
-        const uint32_t box[4] = {vipir::MG_BK, ct, 4 / cg, 1};
-        return make_tmap_nd(&p->tm_c, p->d_cp, 4, dims, str, box);
-    }
+    return VIPIR_OK;
 }
 
-template <int CG>
-int launch_modgemm(vipir_modgemm_plan* p, cudaStream_t st) {
-    auto kern = vipir::modgemm_i8_kernel<CG>;
+// C limb planes [P][4][ncols][Kp]; box = 128 B x ct columns x (4/cg) planes of one problem
+int ensure_c_planes(vipir_modgemm_plan* p) {
+    if (p->d_cp) return VIPIR_OK;
+    if (cudaMalloc(&p->d_cp, p->cp_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return VIPIR_ERR_ALLOC;
+    }
+    const uint64_t dims[4] = {p->Kp, p->ncols, 4, p->P};
+    const uint64_t str[3] = {p->Kp, (uint64_t)p->Kp * p->ncols, 4ull * p->Kp * p->ncols};
+    const uint32_t box[4] = {vipir::MG_BK, p->mg.ct, 4 / p->cg, 1};
+    return make_tmap_nd(&p->tm_c, p->d_cp, 4, dims, str, box);
+}
+
+template <int CG, bool FUSED>
+int launch_modgemm(vipir_modgemm_plan* p, const vipir::ModGemmParams& g, cudaStream_t st) {
+    auto kern = vipir::modgemm_i8_kernel<CG, FUSED>;
     static thread_local uint64_t attr_set = 0;  // bit d: done on device d
     if (attr_needed(attr_set)) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
@@ -138,7 +174,7 @@ int launch_modgemm(vipir_modgemm_plan* p, cudaStream_t st) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p->grid);
     cfg.blockDim = dim3(vipir::MG_THREADS);
-    cfg.dynamicSmemBytes = p->smem_bytes;
+    cfg.dynamicSmemBytes = FUSED ? p->smem_bytes_fused : p->smem_bytes;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -147,7 +183,7 @@ int launch_modgemm(vipir_modgemm_plan* p, cudaStream_t st) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_h, p->tm_c, p->mg));
+    CK(cudaLaunchKernelEx(&cfg, kern, p->tm_h, FUSED ? p->tm_c_raw : p->tm_c, g));
     return VIPIR_OK;
 }
 
@@ -178,7 +214,8 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
     *out = nullptr;
     if (tune) {
         if (tune->cta_group > 2 || tune->tile_cols > 64 || tune->tile_cols % 8 != 0 || tune->b_stages == 1 ||
-            tune->b_stages > 4 || (tune->a_stages != 0 && tune->a_stages < 4) || tune->a_stages > 24)
+            tune->b_stages > 4 || (tune->a_stages != 0 && tune->a_stages < 4) || tune->a_stages > 24 ||
+            tune->c_split > 2 || tune->r_stages == 1 || tune->r_stages > 4)
             return VIPIR_ERR_INVALID_ARG;
         for (uint32_t r : tune->reserved)
             if (r != 0) return VIPIR_ERR_INVALID_ARG;
@@ -215,14 +252,27 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
     // enough for its shared-memory traffic to matter
     p->cg = (M > 128 && ncols >= 16) ? 2u : 1u;  // measured: pairs win from 16 columns up (8 clients: 2.64 -> 2.55 ms)
     if (p->tune.cta_group) p->cg = p->tune.cta_group;
+    // One kernel (C split into limbs inside the products kernel) or two (a splitter pre-pass writes C's limb planes).
+    // The raw-C tensor map needs 16-byte row strides: K % 4 == 0 (the paper's n = 1280).  Measured at the paper's shape
+    // (sustained, same run): 64 columns 4.95 against 5.6 ms, 16 columns 3.01 against 2.93 ms, 2 columns 2.51 against
+    // 2.42 ms -- the pre-pass costs 2 * 4 bytes per word of C, the fused form a longer dependency chain per k-atom:
+    // fused from 32 columns up.
+    if (p->tune.c_split == 2 && K % 4 != 0) {
+        delete p;
+        return VIPIR_ERR_UNSUPPORTED;
+    }
+    p->fused = p->tune.c_split ? p->tune.c_split == 2 : (K % 4 == 0 && ncols >= 32);
     p->hp_bytes = p->P * M * 4ull * p->Kp;
     p->cp_bytes = p->P * 4ull * ncols * p->Kp;
-    if (cudaMalloc(&p->d_hp, p->hp_bytes) != cudaSuccess || cudaMalloc(&p->d_cp, p->cp_bytes) != cudaSuccess) {
+    // the C limb planes are only needed by the two-kernel form: allocated here when that is the plan's form,
+    // else on the first vipir_modgemm_split_c
+    if (cudaMalloc(&p->d_hp, p->hp_bytes) != cudaSuccess) {
         cudaGetLastError();
         vipir_modgemm_destroy(p);
         return VIPIR_ERR_ALLOC;
     }
     int rc = plan_modgemm(p);
+    if (rc == VIPIR_OK && !p->fused) rc = ensure_c_planes(p);
     if (rc != VIPIR_OK) {
         vipir_modgemm_destroy(p);
         return rc;
@@ -240,24 +290,55 @@ int vipir_modgemm_set_h(vipir_modgemm_plan* p, const uint32_t* d_H, void* cuda_s
 
 int vipir_modgemm_split_c(vipir_modgemm_plan* p, const uint32_t* d_C, void* cuda_stream) {
     if (!p || !d_C || (reinterpret_cast<uintptr_t>(d_C) & 15)) return VIPIR_ERR_INVALID_ARG;
+    int rc = ensure_c_planes(p);
+    if (rc != VIPIR_OK) return rc;
     return launch_mg_split<false>(d_C, p->d_cp, p->P * p->ncols, p->ncols, p->K, p->Kp,
                                   static_cast<cudaStream_t>(cuda_stream));
 }
 
-int vipir_modgemm_products(vipir_modgemm_plan* p, const uint32_t* d_G, uint32_t* d_Out, void* cuda_stream) {
+namespace {
+int check_products_args(const vipir_modgemm_plan* p, const uint32_t* d_G, const uint32_t* d_Out) {
     if (!p || !d_Out || (p->gcols > 0 && !d_G)) return VIPIR_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(d_Out) & 3) || (reinterpret_cast<uintptr_t>(d_G) & 3)) return VIPIR_ERR_INVALID_ARG;
     if (!p->h_set) return VIPIR_ERR_INVALID_ARG;
-    p->mg.G = d_G;
-    p->mg.out = d_Out;
+    return VIPIR_OK;
+}
+}  // namespace
+
+int vipir_modgemm_products(vipir_modgemm_plan* p, const uint32_t* d_G, uint32_t* d_Out, void* cuda_stream) {
+    int rc = check_products_args(p, d_G, d_Out);
+    if (rc != VIPIR_OK) return rc;
+    if (!p->d_cp) return VIPIR_ERR_INVALID_ARG;  // no limb planes yet: vipir_modgemm_split_c first
+    vipir::ModGemmParams g = p->mg;  // per-call values go into a copy
+    g.G = d_G;
+    g.out = d_Out;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    return p->cg == 2 ? launch_modgemm<2>(p, st) : launch_modgemm<1>(p, st);
+    return p->cg == 2 ? launch_modgemm<2, false>(p, g, st) : launch_modgemm<1, false>(p, g, st);
 }
 
 int vipir_modgemm(vipir_modgemm_plan* p, const uint32_t* d_C, const uint32_t* d_G, uint32_t* d_Out, void* cuda_stream) {
-    int rc = vipir_modgemm_split_c(p, d_C, cuda_stream);
+    if (!p || !d_C || (reinterpret_cast<uintptr_t>(d_C) & 15)) return VIPIR_ERR_INVALID_ARG;
+    if (!p->fused) {
+        int rc = vipir_modgemm_split_c(p, d_C, cuda_stream);
+        if (rc != VIPIR_OK) return rc;
+        return vipir_modgemm_products(p, d_G, d_Out, cuda_stream);
+    }
+    int rc = check_products_args(p, d_G, d_Out);
     if (rc != VIPIR_OK) return rc;
-    return vipir_modgemm_products(p, d_G, d_Out, cuda_stream);
+    if (p->tm_c_raw_for != d_C) {
+        // the caller's C as it lies: [P][ncols][K] u32; box = 32 words x ct columns of one problem, 128B swizzle
+        const uint64_t dims[3] = {p->K, p->ncols, p->P};
+        const uint64_t str[2] = {4ull * p->K, 4ull * p->K * p->ncols};
+        const uint32_t box[3] = {32, p->mg.ct, 1};
+        rc = make_tmap_nd(&p->tm_c_raw, d_C, 3, dims, str, box, CU_TENSOR_MAP_DATA_TYPE_UINT32);
+        if (rc != VIPIR_OK) return rc;
+        p->tm_c_raw_for = d_C;
+    }
+    vipir::ModGemmParams g = p->mg_fused;
+    g.G = d_G;
+    g.out = d_Out;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    return p->cg == 2 ? launch_modgemm<2, true>(p, g, st) : launch_modgemm<1, true>(p, g, st);
 }
 
 int vipir_modgemm_info(const vipir_modgemm_plan* p, vipir_modgemm_info_t* o) {
@@ -271,14 +352,16 @@ int vipir_modgemm_info(const vipir_modgemm_plan* p, vipir_modgemm_info_t* o) {
     o->m_tiles = p->mg.m_tiles;
     o->n_tiles = p->mg.n_tiles;
     o->n_chunks = p->mg.n_chunks;
-    o->a_stages = p->mg.a_stages;
-    o->b_stages = p->mg.b_stages;
-    o->acc_stages = p->mg.acc_stages;
-    o->smem_bytes = p->smem_bytes;
+    const vipir::ModGemmParams& g = p->fused ? p->mg_fused : p->mg;
+    o->a_stages = g.a_stages;
+    o->b_stages = g.b_stages;
+    o->acc_stages = g.acc_stages;
+    o->smem_bytes = p->fused ? p->smem_bytes_fused : p->smem_bytes;
     o->grid = p->grid;
-    o->launches = 2;
+    o->launches = p->fused ? 1 : 2;
+    o->fused_split = p->fused ? 1 : 0;
     o->h_limb_bytes = p->hp_bytes;
-    o->c_limb_bytes = p->cp_bytes;
+    o->c_limb_bytes = p->d_cp ? p->cp_bytes : 0;
     return VIPIR_OK;
 }
 

@@ -28,9 +28,25 @@
 //   warp 0   TMA producer: per k-atom (128 k) one B box (4 limb planes x ct columns x 128 B) and
 //            four A boxes (128 rows x 128 B, one per H limb) into two mbarrier rings;
 //   warp 1   MMA issuer (one thread): per A box four tcgen05.mma (K = 32 each);
-//   warp 2   TMEM allocator;   warps 4-11 epilogue: tcgen05.ld, recombine in u64 (shifts for the
+//   warp 2   TMEM allocator;   warps 2-3 (FUSED) converters, see below;
+//   warps 4-11 epilogue: tcgen05.ld, recombine in u64 (shifts for the
 //            low four sums, 2^(8s) mod q weights for the high three), + G, one Barrett reduction,
 //            store (coalesced over rows).
+//
+// FUSED (the default whenever K % 4 == 0): the limb split of C -- the paper fuses its prmt decomposition into
+// the GEMM kernel too -- happens inside this kernel instead of a pre-pass that writes and re-reads
+// 4 bytes per word of C.  The producer brings the RAW u32 words of the C tile by TMA (four 32-word x ct-column
+// boxes per k-atom, 128B-swizzled so that a thread's 64-byte run reads conflict-free), two converter warps
+// byte-transpose them with prmt (split_limbs.cuh) and write the limb planes straight into the swizzled K-major
+// B operand slot the tensor core reads; fence.proxy.async + an mbarrier arrival hand the slot to the MMA issuer.
+// With CTA pairs (CTA c stages limb planes 2c, 2c + 1 of the whole tile) each CTA reads the whole raw tile (the
+// second read hits L2) and converts its two planes, so every write stays in the CTA's own shared memory.  The
+// converters hand a slot over with fence.proxy.async.shared::cta and an arrival on their OWN CTA's barrier; for
+// the peer CTA the otherwise idle warp 1 forwards that arrival to the leader's barrier with one cluster-scope
+// release per k-atom.  (Measured alternatives: a release.cluster arrival in the converters
+// themselves, or halving the raw tile per CTA and writing the peer's planes through distributed shared memory,
+// cost a GPU-scope membar per converter warp and k-atom -- 1.3-1.5x slower than the two-kernel form; TMA cannot
+// gather the 16-bit half of every word, element strides do not apply to dimension 0.)
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -44,6 +60,7 @@ constexpr int MG_BM = 128;      // rows per CTA
 constexpr int MG_BK = 128;      // k per atom = bytes per limb-plane row segment (one 128B swizzle row)
 constexpr int MG_UMMA_K = 32;
 constexpr int MG_EPI_WARPS = 8;  // two per TMEM lane quarter, splitting the column groups
+constexpr int MG_CONV_WARPS = 2; // warps 2 and 3: raw C words -> limb planes in shared memory (FUSED)
 constexpr int MG_THREADS = 32 * (4 + MG_EPI_WARPS);
 constexpr int MG_A_BYTES = MG_BM * MG_BK;  // 16 KiB: one H limb of one k-atom
 constexpr int MG_ZERO_BYTES = 1024;        // all-zero A operand (one 8-row swizzle atom, aliased by SBO = 0)
@@ -59,6 +76,8 @@ struct ModGemmParams {
     uint32_t atoms;    // k-atoms = Kp / 128
     uint32_t atoms_per_chunk, n_chunks;
     uint32_t a_stages, b_stages, b_stage_bytes;  // per CTA
+    uint32_t r_stages, r_stage_bytes;            // FUSED: ring of raw C tiles (ct columns x 128 words as four 32-word
+                                                 // boxes), per CTA
     uint32_t tmem_cols, acc_stages;
     uint32_t idesc;
     uint32_t moduli[MG_MAX_MODULI];
@@ -123,19 +142,23 @@ __device__ __forceinline__ uint64_t make_smem_desc_zero(uint32_t saddr) {
     return d;
 }
 
-template <int CG>
+// tmB: the C limb planes (FUSED = false) or the raw u32 words of C (FUSED = true)
+template <int CG, bool FUSED>
 __global__ void __launch_bounds__(MG_THREADS, 1)
 modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, ModGemmParams p) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* sA_ring = smem;
     uint8_t* sB_ring = sA_ring + (size_t)p.a_stages * MG_A_BYTES;
-    uint8_t* sZero = sB_ring + (size_t)p.b_stages * p.b_stage_bytes;
+    uint8_t* sR_ring = sB_ring + (size_t)p.b_stages * p.b_stage_bytes;
+    uint8_t* sZero = sR_ring + (FUSED ? (size_t)p.r_stages * p.r_stage_bytes : 0);
     uint64_t* fullA = reinterpret_cast<uint64_t*>(sZero + MG_ZERO_BYTES);
     uint64_t* emptyA = fullA + p.a_stages;
     uint64_t* fullB = emptyA + p.a_stages;
     uint64_t* emptyB = fullB + p.b_stages;
-    uint64_t* tmem_full = emptyB + p.b_stages;  // [2]
+    uint64_t* fullR = emptyB + p.b_stages;
+    uint64_t* emptyR = fullR + (FUSED ? p.r_stages : 0);
+    uint64_t* tmem_full = emptyR + (FUSED ? p.r_stages : 0);  // [2]
     uint64_t* tmem_empty = tmem_full + 2;       // [2]
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
 
@@ -161,9 +184,15 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             ptx::mbar_init(&emptyA[s], 1);
         }
         for (uint32_t s = 0; s < p.b_stages; ++s) {
-            ptx::mbar_init(&fullB[s], 1);
+            // FUSED: the slot is filled by this CTA's converter warps; the leader also counts the peer's forwarder
+            ptx::mbar_init(&fullB[s], FUSED ? MG_CONV_WARPS + ((CG == 2 && rank == 0) ? 1 : 0) : 1);
             ptx::mbar_init(&emptyB[s], 1);
         }
+        if constexpr (FUSED)
+            for (uint32_t s = 0; s < p.r_stages; ++s) {
+                ptx::mbar_init(&fullR[s], 1);
+                ptx::mbar_init(&emptyR[s], MG_CONV_WARPS);
+            }
         for (uint32_t a = 0; a < 2; ++a) {
             ptx::mbar_init(&tmem_full[a], 1);
             ptx::mbar_init(&tmem_empty[a], MG_EPI_WARPS * CG);
@@ -191,6 +220,22 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 const uint32_t mt = rem / p.n_tiles, nt = rem % p.n_tiles;
                 const int32_t row0 = (int32_t)((mt * CG + rank) * MG_BM);
                 for (uint32_t a = 0; a < p.atoms; ++a) {
+                    if constexpr (FUSED) {
+                        // the raw words of the C tile (every CTA its own copy): four 32-word k-blocks
+                        ptx::mbar_wait(&emptyR[sb], pb ^ 1);
+                        __syncwarp();
+                        uint8_t* dR = sR_ring + (size_t)sb * p.r_stage_bytes;
+                        if (ptx::elect_one()) {
+                            ptx::mbar_arrive_expect_tx(&fullR[sb], p.r_stage_bytes);
+#pragma unroll
+                            for (uint32_t kb = 0; kb < 4; ++kb)
+                                ptx::tma_load_3d(dR + kb * (p.r_stage_bytes / 4), &tmB, &fullR[sb],
+                                                 (int32_t)(a * MG_BK + kb * 32), (int32_t)(nt * p.ct), (int32_t)prob,
+                                                 ptx::kEvictNormal);
+                        }
+                        __syncwarp();
+                        if (++sb == p.r_stages) { sb = 0; pb ^= 1; }
+                    } else {
                     ptx::mbar_wait(&emptyB[sb], pb ^ 1);
                     __syncwarp();
                     uint8_t* dB = sB_ring + (size_t)sb * p.b_stage_bytes;
@@ -209,6 +254,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     }
                     __syncwarp();
                     if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
+                    }
 #pragma unroll 1
                     for (uint32_t i = 0; i < 4; ++i) {
                         ptx::mbar_wait(&emptyA[sa], pa ^ 1);
@@ -248,7 +294,9 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     const uint32_t a_end = min(p.atoms, a_begin + p.atoms_per_chunk);
                     const uint32_t tacc = tmem_base + as * acc_cols;
                     for (uint32_t a = a_begin; a < a_end; ++a) {
-                        ptx::mbar_wait(&fullB[sb], pb);
+                        // FUSED pairs: the peer's converter warps arrive on this barrier too (cluster-scope acquire)
+                        if constexpr (FUSED && CG == 2) ptx::mbar_wait_cluster(&fullB[sb], pb);
+                        else ptx::mbar_wait(&fullB[sb], pb);
                         ptx::tc_fence_after();
                         const uint64_t dB = make_smem_desc(ptx::smem_u32(sB_ring + (size_t)sb * p.b_stage_bytes));
 #pragma unroll 1
@@ -284,6 +332,62 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                         if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
                     }
                 }
+            }
+        } else if constexpr (FUSED && CG == 2) {
+            // ===== rank 1's warp 1 (the MMA issuer sits in rank 0): forwards "this CTA's operand half is written" =====
+            uint32_t sb = 0, pb = 0;
+            for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+                for (uint32_t a = 0; a < p.atoms; ++a) {
+                    ptx::mbar_wait(&fullB[sb], pb);
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive_cluster(&fullB[sb], 0);  // release at cluster scope
+                    if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
+                }
+            }
+        }
+    } else if (FUSED && (warp == 2 || warp == 3)) {
+        // ===== converter warps: raw C words -> this CTA's limb planes in the B operand slot =====
+        const uint32_t tid = (warp - 2) * 32 + lane;
+        uint32_t sr = 0, pr = 0, sb = 0, pb = 0;
+        for (uint32_t u = unit0; u < n_units; u += unit_stride) {
+            for (uint32_t a = 0; a < p.atoms; ++a) {
+                ptx::mbar_wait(&fullR[sr], pr);
+                ptx::mbar_wait(&emptyB[sb], pb ^ 1);  // the MMAs that read this operand slot are done
+                ptx::tc_fence_after();
+                const uint8_t* raw = sR_ring + (size_t)sr * p.r_stage_bytes;
+                uint8_t* dst = sB_ring + (size_t)sb * p.b_stage_bytes;
+                // one item = 16 consecutive k of one column, one 16-byte chunk per limb plane out.  Eight neighbouring
+                // lanes take eight neighbouring columns (ct % 8 == 0): their 16-byte accesses land on eight different
+                // chunk positions of the 128B swizzle, in the raw tile and in the operand
+                for (uint32_t idx = tid; idx < 8 * p.ct; idx += 32 * MG_CONV_WARPS) {
+                    const uint32_t r = idx % p.ct, kh = idx / p.ct, sw = r & 7;  // kh: which 16 k of the atom's 128
+                    const uint8_t* src = raw + (kh >> 1) * (p.r_stage_bytes / 4) + r * 128;  // 32 words a box
+                    uint8_t* d0 = dst + r * 128 + ((kh ^ sw) << 4);
+                    uint32_t L[4][4];
+#pragma unroll
+                    for (uint32_t w = 0; w < 4; ++w) {
+                        const uint4 v = *reinterpret_cast<const uint4*>(src + (((4 * (kh & 1) + w) ^ sw) << 4));
+                        byte_transpose4(v.x, v.y, v.z, v.w, L[w]);
+                    }
+                    if constexpr (CG == 1) {
+#pragma unroll
+                        for (uint32_t j = 0; j < 4; ++j)
+                            *reinterpret_cast<uint4*>(d0 + j * p.ct * 128) = make_uint4(L[0][j], L[1][j], L[2][j], L[3][j]);
+                    } else {  // this CTA stages planes 2*rank and 2*rank + 1
+                        *reinterpret_cast<uint4*>(d0) = rank ? make_uint4(L[0][2], L[1][2], L[2][2], L[3][2])
+                                                             : make_uint4(L[0][0], L[1][0], L[2][0], L[3][0]);
+                        *reinterpret_cast<uint4*>(d0 + p.ct * 128) = rank ? make_uint4(L[0][3], L[1][3], L[2][3], L[3][3])
+                                                                          : make_uint4(L[0][1], L[1][1], L[2][1], L[3][1]);
+                    }
+                }
+                ptx::fence_proxy_async();  // generic-proxy writes -> visible to the tensor core's async proxy
+                __syncwarp();
+                if (lane == 0) {
+                    ptx::mbar_arrive(&emptyR[sr]);
+                    ptx::mbar_arrive(&fullB[sb]);
+                }
+                if (++sr == p.r_stages) { sr = 0; pr ^= 1; }
+                if (++sb == p.b_stages) { sb = 0; pb ^= 1; }
             }
         }
     } else if (warp >= 4) {

@@ -57,7 +57,7 @@ def test_tuning_domain_is_checked_before_any_device_call(lib):
         tune = vipir.ModGemmTuning(**fields)
         q = (ctypes.c_uint32 * 1)(97)
         return lib.vipir_modgemm_plan_create_tuned(ctypes.byref(h), 1, 2, 128, 128, 8, 0, q, ctypes.byref(tune))
-    for bad in (dict(cta_group=3), dict(tile_cols=12), dict(tile_cols=72), dict(a_stages=3), dict(a_stages=25),
+    for bad in (dict(cta_group=3), dict(tile_cols=12), dict(tile_cols=72), dict(a_stages=3), dict(a_stages=25), dict(c_split=3), dict(r_stages=1), dict(r_stages=5),
                 dict(b_stages=1), dict(b_stages=5)):
         assert mg(**bad) == vipir.ERR_INVALID_ARG, bad
 

@@ -36,9 +36,11 @@ def run_modgemm(H, C, G, moduli, cg=0, ct=0, return_info=False, via_parts=False)
     d_C = torch.from_numpy(np.ascontiguousarray(C).view(np.int32)).cuda()
     d_G = None if G is None else torch.from_numpy(np.ascontiguousarray(G).view(np.int32)).cuda()
     d_O = torch.full((T, NC, ncols, M), -1, dtype=torch.int32, device="cuda")  # poison
+    fusable = K % 4 == 0
     with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli, tuning=tuning) as plan:
         plan.set_h(d_H)
-        del d_H  # the plan owns its own re-laid-out copy
+        assert plan.info["fused_split"] == (1 if fusable and ncols >= 32 else 0)  # the planner's rule (include/vipir.h)
+        assert plan.info["launches"] == 2 - plan.info["fused_split"]
         if via_parts:
             vipir.modgemm_split_c(plan.handle, d_C)
             vipir.modgemm_products(plan.handle, d_G, d_O)
@@ -46,6 +48,22 @@ def run_modgemm(H, C, G, moduli, cg=0, ct=0, return_info=False, via_parts=False)
             plan(d_C, d_G, d_O)
         torch.cuda.synchronize()
         info = plan.info
+    if not via_parts:
+        # the other form of the same plan shape -- one kernel with C split into limbs in shared memory, or the splitter
+        # pre-pass + products -- must give the same words; so every parity case covers both
+        other = dict(tuning, c_split=1 if info["fused_split"] else 2)
+        if info["fused_split"] or fusable:
+            for extra in ({}, {"r_stages": 2}, {"r_stages": 3, "b_stages": 3}) if not info["fused_split"] else ({},):
+                with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli, tuning=dict(other, **extra)) as plan:
+                    assert plan.info["fused_split"] == (0 if info["fused_split"] else 1)
+                    plan.set_h(d_H)
+                    d_O2 = torch.full_like(d_O, -1)
+                    plan(d_C, d_G, d_O2)
+                    torch.cuda.synchronize()
+                    assert torch.equal(d_O, d_O2), f"fused and two-kernel forms differ ({extra})"
+        else:
+            with pytest.raises(vipir.VipirError):  # no fused form for K % 4 != 0
+                vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli, tuning=dict(tuning, c_split=2))
     out = d_O.cpu().numpy().view(np.uint32)
     return (out, info) if return_info else out
 
