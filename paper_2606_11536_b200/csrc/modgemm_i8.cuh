@@ -437,30 +437,29 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 // every group (register moves), which keeps the indices compile-time constants
 #pragma unroll 1
                 for (uint32_t g = half; g < n_groups; g += 2) {
-                    {
+                    // the group's 8 columns of all seven sums at once, then eight independent reductions (computed
+                    // unconditionally so that the compiler interleaves their multiply chains; only the stores are
+                    // guarded), then the stores
+                    uint32_t v[7][8];
 #pragma unroll
-                        for (int hh = 0; hh < 2; ++hh) {
-                            uint32_t v[7][4];
+                    for (int s = 0; s < 7; ++s) ptx::tmem_ld8(tacc + s * p.ct + g * 8, v[s]);
+                    ptx::tmem_ld_wait();
+                    uint32_t res[8];
 #pragma unroll
-                            for (int s = 0; s < 7; ++s) ptx::tmem_ld4(tacc + s * p.ct + g * 8 + hh * 4, v[s]);
-                            ptx::tmem_ld_wait();
+                    for (int e = 0; e < 8; ++e) {
+                        // sum_s 2^(8s) S_s with S_s < 2^31 (one K chunk).  The low four limb sums are combined with
+                        // shifts (< 2^57); the high three are weighted by 2^(8s) mod q < 2^30 (each product < 2^61),
+                        // so the total stays below 2^63 and ONE Barrett reduction per output word remains.
+                        uint64_t x = (uint64_t)v[0][e] + ((uint64_t)v[1][e] << 8) + ((uint64_t)v[2][e] << 16) +
+                                     ((uint64_t)v[3][e] << 24);
+                        x += (uint64_t)v[4][e] * w4 + (uint64_t)v[5][e] * w5 + (uint64_t)v[6][e] * w6;
+                        x += add[0][e];
+                        res[e] = barrett_u64(x, q, bm);
+                    }
 #pragma unroll
-                            for (int e4 = 0; e4 < 4; ++e4) {
-                                const int e = hh * 4 + e4;
-                                const uint32_t col = nt * p.ct + g * 8 + e;
-                                if (col < p.ncols && row_ok) {
-                                    // sum_s 2^(8s) S_s with S_s < 2^31 (one K chunk).  The low four limb
-                                    // sums are combined with shifts (< 2^57); the high three are weighted
-                                    // by 2^(8s) mod q < 2^30 (each product < 2^61), so the total stays
-                                    // below 2^63 and ONE Barrett reduction per output word remains.
-                                    uint64_t x = (uint64_t)v[0][e4] + ((uint64_t)v[1][e4] << 8) +
-                                                 ((uint64_t)v[2][e4] << 16) + ((uint64_t)v[3][e4] << 24);
-                                    x += (uint64_t)v[4][e4] * w4 + (uint64_t)v[5][e4] * w5 + (uint64_t)v[6][e4] * w6;
-                                    x += add[0][e];
-                                    Op[(uint64_t)col * p.M] = barrett_u64(x, q, bm);
-                                }
-                            }
-                        }
+                    for (int e = 0; e < 8; ++e) {
+                        const uint32_t col = nt * p.ct + g * 8 + e;
+                        if (col < p.ncols && row_ok) Op[(uint64_t)col * p.M] = res[e];
                     }
 #pragma unroll
                     for (int gi = 0; gi < 3; ++gi)
