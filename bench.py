@@ -1,16 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- the VIPIR database scan on B200, measured.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--all]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--paper] [--modgemm] [--pipeline]
 
 Headline (BASELINE.json `metric`: "DB GB/s scanned & TOPS, % of HBM/INT8-TC roofline; 16 GiB u8
 DB, batch 1/256"): one STEP is one pass of the whole hot path -- query-limb split + scan (one
 fused kernel at batch 1), through the C ABI (vipir_dbmul) -- over one batch of synthetic queries against the
 16 GiB u8 database of configs[2] (131072 x 131072, q = 2^32, batch 1).  `value` is GB of DB
 scanned per second with all inputs resident in HBM; `e2e` is the same through vipir_dbmul_host
-with the query in / the answer out of pinned HOST memory inside the timed region.  The batched
-tensor-core regime (configs[3], 4 GiB, batch 256) and the other configs are measured in the
-same run and reported under "batched" / "configs" of the same JSON line.
+with the query in / the answer out of pinned HOST memory inside the timed region.
+
+In the same JSON line (N = 1):
+  "batched"   configs[3] (4 GiB, batch 256) on the tensor cores: sustained step (1 s settle) and burst, its own
+              e2e through vipir_dbmul_host (64 MiB in, 64 MiB out per step), and a tensor roofline against the
+              int8 MMA ceiling measured live (ceilings/ceilings.cu: a pure tcgen05.mma.kind::i8 loop, burst and
+              sustained), with the nominal 4.5 POP/s and the 2 x measured-bf16 fractions beside it
+  "configs"   every BASELINE.json config; each tensor-regime config as `ms_per_step` (sustained) and
+              `ms_per_step_burst`
+  "modgemm", "ntt"   the ring-packing kernels at the paper's 64 GiB hybrid shape for 32
+              clients, each with its roofline (--modgemm adds 1 and 8 clients and the offline H transform)
+  "cpu_baseline"   the oracle on the host cores: median of 100 passes over the first 8192 rows of the headline
+              DB -- the sample and procedure --impl reference uses, so the two agree
 
 The DB (16 GiB) is far larger than the 126 MB L2, so no L2 flush is needed between steps.
 N > 1 (torchrun): the path shards by DB rows with no data-path collective (each

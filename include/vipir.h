@@ -32,8 +32,12 @@
  *
  * Execution: vipir_dbmul only ENQUEUES work on `cuda_stream` (a cudaStream_t / CUstream passed
  * as void*, NULL = legacy default stream): no host synchronisation, no allocation.  One plan
- * must not be in flight on two streams at once (shared workspace).  All kernels are sm_100a;
- * there is no fallback of any kind.
+ * must not be in flight on two streams at once, nor be used from two host threads at once: it
+ * owns one limb-plane workspace, one set of staging buffers and cached tensor maps.  (Per-call
+ * values -- the answer pointer, the modulus-switch and signedness flags in effect -- are passed
+ * to the kernels by value; the planned parameters are never rewritten by a call.)  A server
+ * that overlaps requests makes one plan per stream.  All kernels are sm_100a; there is no
+ * fallback of any kind.
  *
  * Errors: every entry point returns a vipir_status (0 = OK) and never throws or aborts.
  */

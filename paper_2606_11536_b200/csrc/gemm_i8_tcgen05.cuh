@@ -48,7 +48,10 @@
 // global memory before its first read-modify-write.  Group ids are tickets drawn from an atomic
 // counter, a group only ever waits for lower tickets, and every group works through its
 // producing items (the tail of its range) first, so the waits cannot deadlock whatever order the
-// hardware starts the CTAs in; the last group to finish resets the counters for the next launch.
+// hardware starts the CTAs in -- nor when another kernel holds some SMs and part of the grid starts
+// late: a ticket is drawn by a CTA that is already running, and a running CTA is never descheduled
+// before it exits, so every lower ticket a group can wait for belongs to a group that is resident and
+// making progress; the last group to finish resets the counters for the next launch.
 #pragma once
 #include <cstdint>
 #include <cuda.h>

@@ -238,3 +238,15 @@ int main(void) {
                     "-o", str(exe), str(so), f"-Wl,-rpath,{so.parent}"], check=True)
     out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
     assert "c abi ok" in out
+
+
+def test_ceilings_library_loads_and_exports_its_entry_points():
+    """bench.py's measured ceilings (ceilings/libvipir_ceilings.so: bench-only, not product code)."""
+    from paper_2606_11536_b200 import ceilings
+    lib = ceilings._load()
+    for name in ("vipir_ceiling_mma_i8", "vipir_ceiling_butterflies"):
+        assert hasattr(lib, name), name
+    # nothing of the product links or loads it
+    for f in (ROOT / "paper_2606_11536_b200" / "csrc").glob("*.cu*"):
+        assert "ceilings" not in f.read_text(), f
+    assert "ceilings" not in (ROOT / "paper_2606_11536_b200" / "vipir.py").read_text()
