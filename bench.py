@@ -487,9 +487,10 @@ def run_pipeline(B, steps, warmup, offline_hint=False):
         ms_mg = time_events(lambda: mg(d_C, d_G, d_O), steps, warmup, stream) / steps
         bad = ntt.bad_input()
         regime = scan.info["regime_name"]
+        n_kernels = scan.info["launches"] + 1 + mg.info["launches"]
     return {"workload": f"64 GiB u8 DB 2^20 x 2^16, B = {B}; N = 4096, D_r = 256, n = 1280, 3 RNS primes",
             "ms_per_batch": ms, "queries_per_s": B / ms * 1e3, "ms_scan": ms_scan, "ms_ntt_G": ms_ntt,
-            "ms_modgemm": ms_mg, "scan_regime": regime, "kernels_per_batch": 5, "ntt_bad_input": bad,
+            "ms_modgemm": ms_mg, "scan_regime": regime, "kernels_per_batch": n_kernels, "ntt_bad_input": bad,
             "resident_GB": (rows * cols + 4.0 * T * NC * M * 1280) / 1e9, "offline": offline}
 
 
