@@ -164,7 +164,7 @@ __host__ __device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t
 
 // f(unit, chunk, must_wait): must_wait marks the first item of a head segment -- the chunks before
 // it were (or are being) accumulated into the answer by another group.
-// (also instantiated with a host lambda by vipir_debug_work_items: silence the host-call-from-HD diagnostic)
+// (also instantiated with a host lambda by vipir_testing_work_items: silence the host-call-from-HD diagnostic)
 #pragma nv_diag_suppress 20013
 template <class F>
 __host__ __device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f) {
