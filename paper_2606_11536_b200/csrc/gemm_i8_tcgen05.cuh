@@ -438,60 +438,72 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         uint32_t w[NL == 2 ? 4 * LC : 1];  // the D_hi sub-tile's sums for the same row
                         if constexpr (NL == 2) ptx::tmem_ld16(tacc + p.bn + g * (4 * LC), w);
                         ptx::tmem_ld_wait();
+                        if constexpr (PRIME) {
+                            // the four reductions computed unconditionally, so that the compiler interleaves their
+                            // multiply chains; only the stores are guarded (a tile's tail columns reduce garbage that
+                            // is never stored: the modulus index is clamped)
+                            uint32_t val[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const uint32_t q = nt * p.qt + g * 4 + i;
+                                const uint32_t t = min(q / p.batch, p.n_moduli - 1u);
+                                const uint32_t pm = p.moduli[t];
+                                if constexpr (NL == 2) {
+                                    // unsigned; each sum < 2^31, so x < 2^63.1
+                                    uint64_t x = 0;
+#pragma unroll
+                                    for (int s = 0; s < LC; ++s)
+                                        x += ((uint64_t)v[i * LC + s] + ((uint64_t)w[i * LC + s] << 8)) << (8 * s);
+                                    val[i] = barrett_u64(x, pm, p.barrett[t]);
+                                } else if constexpr (LC == 4) {
+                                    // every |P_s| < 2^31 (R7), so the s32 reading is exact for u8 and s8
+                                    // DBs alike and |x| < 2^56; a negative x reduces as p - (|x| mod p)
+                                    int64_t x = 0;
+#pragma unroll
+                                    for (int s = 0; s < LC; ++s) x += (int64_t)(int32_t)v[i * LC + s] << (8 * s);
+                                    const bool neg = x < 0;
+                                    uint32_t r = barrett_u64((uint64_t)(neg ? -x : x), pm, p.barrett[t]);
+                                    if (neg && r != 0) r = pm - r;
+                                    val[i] = r;
+                                } else {
+                                    uint64_t x = 0;  // u16 DB (never signed): up to 2^63 * 1.004
+#pragma unroll
+                                    for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
+                                    val[i] = barrett_u64(x, pm, p.barrett[t]);
+                                }
+                                if (!first) {
+                                    val[i] += old[gg * 4 + i];
+                                    if (val[i] >= pm) val[i] -= pm;
+                                }
+                            }
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const uint32_t q = nt * p.qt + g * 4 + i;
+                                if (q < p.nq && row_ok) obase[(uint64_t)q * p.rows + row] = val[i];
+                            }
+                        } else {
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             const uint32_t q = nt * p.qt + g * 4 + i;
                             if (q < p.nq && row_ok) {
                                 uint32_t* dst = obase + (uint64_t)q * p.rows + row;
-                                if constexpr (!PRIME) {
-                                    // shifts, wrap mod 2^32 (an s = 4 column would vanish)
-                                    uint32_t val =
-                                        v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
-                                    if constexpr (NL == 2)  // D = D_lo + 2^8 D_hi; the 2^32 term of w[3] vanishes
-                                        val += (w[i * LC] << 8) + (w[i * LC + 1] << 16) + (w[i * LC + 2] << 24);
-                                    if (ms_final) {
-                                        if (!first) val += old[gg * 4 + i];
-                                        *dst = modswitch_word(val, p.ms_bits);
-                                    } else if (first) {
-                                        *dst = val;
-                                    } else if (redirect) {
-                                        *dst = val + old[gg * 4 + i];
-                                    } else {
-                                        asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
-                                    }
-                                } else {
-                                    const uint32_t t = q / p.batch;
-                                    const uint32_t pm = p.moduli[t];
-                                    uint32_t val;
-                                    if constexpr (NL == 2) {
-                                        // unsigned; each sum < 2^31, so x < 2^63.1
-                                        uint64_t x = 0;
-#pragma unroll
-                                        for (int s = 0; s < LC; ++s)
-                                            x += ((uint64_t)v[i * LC + s] + ((uint64_t)w[i * LC + s] << 8)) << (8 * s);
-                                        val = barrett_u64(x, pm, p.barrett[t]);
-                                    } else if constexpr (LC == 4) {
-                                        // every |P_s| < 2^31 (R7), so the s32 reading is exact for u8 and s8
-                                        // DBs alike and |x| < 2^56; a negative x reduces as p - (|x| mod p)
-                                        int64_t x = 0;
-#pragma unroll
-                                        for (int s = 0; s < LC; ++s) x += (int64_t)(int32_t)v[i * LC + s] << (8 * s);
-                                        const bool neg = x < 0;
-                                        val = barrett_u64((uint64_t)(neg ? -x : x), pm, p.barrett[t]);
-                                        if (neg && val != 0) val = pm - val;
-                                    } else {
-                                        uint64_t x = 0;  // u16 DB (never signed): up to 2^63 * 1.004
-#pragma unroll
-                                        for (int s = 0; s < LC; ++s) x += (uint64_t)v[i * LC + s] << (8 * s);
-                                        val = barrett_u64(x, pm, p.barrett[t]);
-                                    }
-                                    if (!first) {
-                                        val += old[gg * 4 + i];
-                                        if (val >= pm) val -= pm;
-                                    }
+                                // shifts, wrap mod 2^32 (an s = 4 column would vanish)
+                                uint32_t val =
+                                    v[i * LC] + (v[i * LC + 1] << 8) + (v[i * LC + 2] << 16) + (v[i * LC + 3] << 24);
+                                if constexpr (NL == 2)  // D = D_lo + 2^8 D_hi; the 2^32 term of w[3] vanishes
+                                    val += (w[i * LC] << 8) + (w[i * LC + 1] << 16) + (w[i * LC + 2] << 24);
+                                if (ms_final) {
+                                    if (!first) val += old[gg * 4 + i];
+                                    *dst = modswitch_word(val, p.ms_bits);
+                                } else if (first) {
                                     *dst = val;
+                                } else if (redirect) {
+                                    *dst = val + old[gg * 4 + i];
+                                } else {
+                                    asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
                                 }
                             }
+                        }
                         }
                     }
                 }
