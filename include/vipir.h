@@ -154,7 +154,9 @@ typedef struct {
     uint32_t tile_queries;   /* MMA: query vectors per N tile (a multiple of 4; of 16 when limb_cols == 5), <= 128 */
     uint32_t k_atoms;        /* MMA: 128-byte k-atoms per pipeline stage, 1..8 (lowered until two stages fit) */
     uint32_t stages;         /* shared-memory ring depth: MMA 2..12 (at most what fits), GEMV 2..6 */
-    uint32_t min_chunks;     /* MMA: cut K into at least this many chunks (finer work items; <= number of k-atoms) */
+    uint32_t min_chunks;     /* MMA: cut K into this many equal chunks of whole k-atoms instead of the fewest that respect the
+                                int32 bound (finer work items; <= number of k-atoms; fewer when the k-atoms do not divide
+                                that way: 6 k-atoms in "4" chunks are 3 chunks of 2) */
     uint32_t separate_split; /* GEMV: 1 = always run the query-limb splitter as its own kernel (two launches) */
     uint32_t whole_units;    /* MMA: 1 = deal the last, partial round of work units out whole, not chunk by chunk */
     uint32_t no_collector;   /* MMA: 1 = the second N half re-reads the DB operand from shared memory */

@@ -219,6 +219,9 @@ int plan_gemm(vipir_plan* p, int cg) {
         if (min_chunks > g.n_chunks) g.n_chunks = min_chunks;
     }
     g.ksteps_per_chunk = ceil_div(g.total_ksteps, g.n_chunks);
+    // equal chunks of ceil(k-atoms / n) can leave the last ones empty when n was forced (6 k-atoms in 4 chunks:
+    // 2 + 2 + 2 + 0), and a chunk without k-atoms would never complete its accumulator: count the chunks that exist
+    g.n_chunks = ceil_div(g.total_ksteps, g.ksteps_per_chunk);
     const uint32_t max_groups = (uint32_t)p->num_sms / cg;
     // M sub-tiles per CTA (gemm_i8_tcgen05.cuh): while the product is HBM-bound every DB byte drags
     // bn / (128 * cg * msub) limb-plane bytes through L2 -> SM with it, and that fill (~8 TB/s on the

@@ -469,6 +469,59 @@ def test_host_entry_point_tensor_regimes(name, rows, cols, batch, bits, moduli, 
         assert_same(d_a.cpu().numpy().view(np.uint32), want)
 
 
+def test_forced_chunk_count_that_does_not_divide_the_k_atoms():
+    """6 k-atoms cut into "4" chunks are three chunks of two (a fourth, empty chunk would never complete: this shape
+    hung the kernel until the planner counted the chunks that exist).  Found by a random soak of the host call."""
+    D, Q = make(81, 742, 736, 28, 8, PRIMES)
+    got, info = run_dbmul(D, Q, PRIMES, M1, return_info=True, tuning=dict(min_chunks=4))
+    assert info["n_chunks"] == 3 and info["k_chunk_bytes"] == 256
+    assert_same(got, oracle.dbmul(D, Q, PRIMES, nthreads=NT))
+    for mc, cols in ((5, 896), (7, 1280), (3, 512)):  # 7 k-atoms / 5, 10 / 7, 4 / 3
+        D, Q = make(82, 300, cols, 9)
+        assert_same(run_dbmul(D, Q, None, M2, tuning=dict(min_chunks=mc)), oracle.dbmul(D, Q, nthreads=NT))
+
+
+def _random_host_case(rng):
+    regime = [M1, M2][int(rng.integers(2))]
+    bits = [8, 8, 16][int(rng.integers(3))]
+    moduli = [None, PRIMES][int(rng.integers(2))]
+    rows = int(rng.integers(1, 700))
+    cols = int(rng.integers(1, 300)) * (16 if bits == 8 else 8)
+    batch = int(rng.integers(1, 70))
+    tune = dict(host_slices=int(rng.integers(1, 5)))
+    if rng.integers(3) == 0:
+        tune["min_chunks"] = int(rng.integers(1, 4))
+    ms = 18 if (moduli is None and rng.integers(3) == 0) else 0
+    return regime, bits, moduli, rows, cols, batch, tune, ms
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_host_entry_point_random_shapes(seed):
+    """Seeded random shapes through the K-sliced host call (ragged rows / K / query vectors, 1-4 slices, forced
+    extra chunks so that slices hold several chunks and leftover units are shared between groups)."""
+    import torch
+    ensure_built()
+    rng = np.random.default_rng(1000 + seed)
+    regime, bits, moduli, rows, cols, batch, tune, ms = _random_host_case(rng)
+    D, Q = make(200 + seed, rows, cols, batch, bits, moduli)
+    want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+    if ms:
+        want = oracle.modswitch(want, ms)
+    T = Q.shape[0]
+    d_db = torch.from_numpy(D.view(np.uint8).reshape(rows, -1)).cuda()
+    h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+    h_a = torch.full((T, batch, rows), -1, dtype=torch.int32).pin_memory()
+    try:
+        plan = vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, tuning=tune)
+    except vipir.VipirError as e:  # an override the shape cannot honour (min_chunks > k-atoms) is refused, not ignored
+        assert e.status == vipir.ERR_UNSUPPORTED and "min_chunks" in tune
+        tune.pop("min_chunks")
+        plan = vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, tuning=tune)
+    with plan:
+        plan.host(d_db, h_q, h_a)
+        assert_same(h_a.numpy().view(np.uint32), want)
+
+
 def test_misaligned_pointers_are_rejected():
     import torch
     ensure_built()
