@@ -467,6 +467,13 @@ def test_host_entry_point_tensor_regimes(name, rows, cols, batch, bits, moduli, 
         plan(d_db, torch.from_numpy(Q.view(np.int32)).cuda(), d_a)
         torch.cuda.synchronize()
         assert_same(d_a.cpu().numpy().view(np.uint32), want)
+    # a fresh plan used at once on a non-blocking side stream (plan-time zeroing of the work counters is complete
+    # when the plan call returns; the copy stream is ordered after the caller's stream)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side), vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, signed, tuning=tune) as plan:
+        pinned.fill_(-1)
+        plan.host(d_db, h_q, pinned[:T * batch * rows])
+        assert_same(pinned[:T * batch * rows].numpy().view(np.uint32).reshape(T, batch, rows), want)
 
 
 def test_forced_chunk_count_that_does_not_divide_the_k_atoms():
