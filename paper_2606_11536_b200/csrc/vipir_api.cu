@@ -645,10 +645,21 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     // copy stream: H2D of slice i's columns of every query vector (a strided copy), its split;  caller's stream:
     // the scan of slice i, which adds to the running sums of the slices before it.  The last slice's last chunk
     // writes the finished words to the host buffer (directly when it is mapped).
-    if (!p->copy_stream) {
-        CK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
-        CK(cudaEventCreateWithFlags(&p->ev_begin, cudaEventDisableTiming));
-        for (uint32_t i = 0; i < kMaxHostSlices; ++i) CK(cudaEventCreateWithFlags(&p->ev_slice[i], cudaEventDisableTiming));
+    if (!p->copy_stream) {  // all of them or none: a later call must not find a stream without its events
+        cudaStream_t cs = nullptr;
+        cudaEvent_t ev[kMaxHostSlices + 1] = {};
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        for (uint32_t i = 0; e == cudaSuccess && i <= kMaxHostSlices; ++i)
+            e = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            for (cudaEvent_t x : ev)
+                if (x) cudaEventDestroy(x);
+            if (cs) cudaStreamDestroy(cs);
+            return cuda_fail(e, "vipir_dbmul_host: copy stream / events");
+        }
+        p->copy_stream = cs;
+        p->ev_begin = ev[kMaxHostSlices];
+        for (uint32_t i = 0; i < kMaxHostSlices; ++i) p->ev_slice[i] = ev[i];
     }
     CK(cudaEventRecord(p->ev_begin, st));  // the staging buffers may still be read by work queued on `st`
     CK(cudaStreamWaitEvent(p->copy_stream, p->ev_begin, 0));
