@@ -15,7 +15,7 @@ struct vipir_modgemm_plan {
     uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
     uint64_t hp_bytes, cp_bytes;
     bool h_set;
-    bool fused;          // vipir_modgemm splits C inside the products kernel (K % 4 == 0): one launch, no C limb planes
+    bool fused;          // vipir_modgemm splits C inside the products kernel (from 32 columns up, K % 4 == 0): one launch
     vipir::ModGemmParams mg, mg_fused;
     uint32_t smem_bytes, smem_bytes_fused, grid;
     CUtensorMap tm_h, tm_c;
@@ -109,7 +109,7 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / q);
     }
     p->smem_bytes = g.a_stages * vipir::MG_A_BYTES + g.b_stages * g.b_stage_bytes + overhead;
-    // the fused kernel: two operand slots, two raw-tile slots (ct columns x 128 words each), the rest to the H ring
+    // the fused kernel: two operand slots, two to four raw-tile slots (ct columns x 128 words each), the rest to the H ring
     p->mg_fused = g;
     if (p->fused) {
         vipir::ModGemmParams& f = p->mg_fused;
