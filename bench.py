@@ -202,6 +202,47 @@ def step_spread(fn, steps, stream):
     return {"median": t[len(t) // 2], "best": t[0], "worst": t[-1]}
 
 
+def two_in_flight(rows, cols, batch, db_bits, moduli, layout, d_db, h_q, d_ref, steps):
+    """A server that overlaps requests makes one plan per stream (include/vipir.h): two host threads, each with its own
+    plan, stream and pinned buffers, call vipir_dbmul_host back to back against the same resident DB -- the copies of one
+    request run beside the scan of the other.  Returns ms per request (all requests / the slower thread's device time,
+    CUDA events on each thread's stream), after both threads have settled for a second."""
+    import torch
+    from paper_2606_11536_b200 import vipir
+    T = h_q.shape[0]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    plans = [vipir.Plan(rows, cols, batch, db_bits, moduli, db_layout=layout) for _ in range(2)]
+    bufs = [(h_q if i == 0 else h_q.clone().pin_memory(), torch.empty((T, batch, rows), dtype=torch.int32).pin_memory())
+            for i in range(2)]
+    ms = [0.0, 0.0]
+    start = threading.Barrier(2)
+
+    def worker(i):
+        torch.cuda.set_device(d_db.device)
+        with torch.cuda.stream(streams[i]):
+            t_end = time.perf_counter() + SETTLE_S
+            while time.perf_counter() < t_end:
+                plans[i].host(d_db, bufs[i][0], bufs[i][1])
+            start.wait()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(streams[i])
+            for _ in range(steps):
+                plans[i].host(d_db, bufs[i][0], bufs[i][1])
+            e1.record(streams[i])
+            streams[i].synchronize()
+            ms[i] = e0.elapsed_time(e1)
+    th = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    for i in range(2):
+        if not torch.equal(bufs[i][1].cuda(), d_ref):
+            raise RuntimeError("two requests in flight: an answer differs from vipir_dbmul's")
+        plans[i].close()
+    return max(ms) / (2 * steps)
+
+
 def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset_bytes=0, spread=False):
     """Times one config on the current device; returns a dict of measurements.  Every config that runs on the tensor
     cores is timed in the power-capped steady state (a 1 s settle loop first: `ms_per_step`, the number of record)
@@ -276,6 +317,8 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
             out["pcie_d2h_GBps"] = h_q.numel() * 4 / (time_events(lambda: h_q.copy_(d_tmp, non_blocking=True), 5, 2, stream) / 5) / 1e6
             if not torch.equal(h_a.cuda(), d_a):
                 raise RuntimeError(f"{name}: vipir_dbmul_host and vipir_dbmul disagree")
+            if tensor:
+                out["e2e_two_in_flight_ms"] = two_in_flight(rows, cols, batch, db_bits, moduli, layout, d_db, h_q, d_a, steps)
             del h_q, h_a, d_tmp
     db_bytes = rows * kb
     nq, lc = info["query_vectors"], info["limb_cols"]
@@ -648,6 +691,12 @@ def run_cuda(args):
                 "e2e": {"ms_per_step": b["e2e_ms"], "int8_TOPS": b["int8_ops"] / b["e2e_ms"] / 1e9,
                         "db_GBps": b["rows"] * b["cols"] / b["e2e_ms"] / 1e6,
                         "ratio_to_device_step": b["e2e_ms"] / b["ms_per_step"],
+                        "two_requests_in_flight": {
+                            "ms_per_request": b["e2e_two_in_flight_ms"],
+                            "ratio_to_device_step": b["e2e_two_in_flight_ms"] / b["ms_per_step"],
+                            "how": "two host threads, each with its own plan, stream and pinned buffers, calling "
+                                   "vipir_dbmul_host back to back on the same resident DB: one request's copies run "
+                                   "beside the other's scan (throughput of a server that overlaps requests)"},
                         "h2d_bytes_per_step": b["h2d_bytes"], "d2h_bytes_per_step": b["d2h_bytes"],
                         "pcie_h2d_GBps": b["pcie_h2d_GBps"], "pcie_d2h_GBps": b["pcie_d2h_GBps"],
                         "how": "vipir_dbmul_host: H2D, limb split and scan pipelined over K slices, the answer "

@@ -529,6 +529,42 @@ def test_host_entry_point_random_shapes(seed):
         assert_same(h_a.numpy().view(np.uint32), want)
 
 
+def test_two_plans_two_threads_two_streams():
+    """One plan per stream (include/vipir.h): two host threads, each with its own plan, side stream and pinned buffers,
+    call vipir_dbmul_host repeatedly against the same resident DB; every answer is the oracle's."""
+    import threading
+    import torch
+    ensure_built()
+    rows, cols, batch = 520, 4112, 40
+    D = inputs.db_rows(95, rows, cols, 8)
+    d_db = torch.from_numpy(D).cuda()
+    Qs = [inputs.query(96 + i, cols, batch) for i in range(2)]
+    wants = [oracle.dbmul(D, Q, nthreads=NT) for Q in Qs]
+    errors = []
+
+    def worker(i):
+        try:
+            torch.cuda.set_device(0)
+            side = torch.cuda.Stream()
+            h_q = torch.from_numpy(Qs[i].view(np.int32)).pin_memory()
+            h_a = torch.full((1, batch, rows), -1, dtype=torch.int32).pin_memory()
+            with torch.cuda.stream(side), vipir.Plan(rows, cols, batch, 8, None, M2, tuning=dict(host_slices=3)) as plan:
+                for _ in range(25):
+                    h_a.fill_(-1)
+                    plan.host(d_db, h_q, h_a)
+                    if not np.array_equal(h_a.numpy().view(np.uint32), wants[i]):
+                        errors.append(f"thread {i}: answer differs")
+                        return
+        except Exception as e:  # noqa: BLE001
+            errors.append(f"thread {i}: {e!r}")
+    th = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errors, errors
+
+
 def test_misaligned_pointers_are_rejected():
     import torch
     ensure_built()
