@@ -17,7 +17,8 @@
 //            planes are laid out so that the LC limb sums of one query are LC adjacent
 //            accumulator columns;
 //   warp 2   TMEM allocator;
-//   warps 4-7 epilogue: tcgen05.ld the accumulators of their lane quarter, recombine limbs
+//   warps 4-11 epilogue (two per TMEM lane quarter, taking alternate batches of 32 query vectors):
+//            tcgen05.ld the accumulators of their lane quarter, recombine limbs
 //            with shifts (wrap mod 2^32) or in u64 + Barrett (prime moduli), and store /
 //            read-modify-write answer[q][row] (coalesced over rows).
 // The K dimension is processed in chunks of <= 32768 bytes (256 k-steps): 255*255*32768 <
@@ -62,7 +63,8 @@ namespace vipir {
 constexpr int GM_BM = 128;           // rows per CTA
 constexpr int GM_BK = 128;           // bytes of K per stage (one 128B swizzle row)
 constexpr int GM_UMMA_K = 32;        // bytes of K per tcgen05.mma.kind::i8
-constexpr int GM_THREADS = 256;
+constexpr int GM_EPI_WARPS = 8;      // two per TMEM lane quarter (a warp reads the 32 lanes of quarter warp % 4)
+constexpr int GM_THREADS = 32 * (4 + GM_EPI_WARPS);
 constexpr int GM_A_BYTES = GM_BM * GM_BK;  // 16384
 constexpr int GM_MAX_MODULI = 4;
 
@@ -230,7 +232,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         for (uint32_t a = 0; a < 2; ++a) {
             ptx::mbar_init(&tmem_full[a], 1);
-            ptx::mbar_init(&tmem_empty[a], 4 * CG);  // one arrival per epilogue warp of every CTA
+            ptx::mbar_init(&tmem_empty[a], GM_EPI_WARPS * CG);  // one arrival per epilogue warp of every CTA
         }
         ptx::fence_barrier_init();
     }
@@ -380,8 +382,9 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             });
         }
     } else if (warp >= 4) {
-        // ===== epilogue warps: lane quarter = warp % 4 =====
+        // ===== epilogue warps: lane quarter = warp % 4; the two warps of a quarter take alternate batches of kPf steps =====
         const uint32_t quarter = warp & 3;
+        const uint32_t half = (warp - 4) >> 2;
         uint32_t acc_it = 0;
         for_each_item(work, [&](uint32_t u, uint32_t c, bool must_wait) {
             const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
@@ -391,10 +394,10 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             ptx::mbar_wait(&tmem_full[as], aphase);
             ptx::tc_fence_after();
             if (must_wait) {
-                // chunks [0, c) of this unit belong to another group: all of its (4 * CG) epilogue
+                // chunks [0, c) of this unit belong to another group: all of its (GM_EPI_WARPS * CG) epilogue
                 // warps must have stored them before this read-modify-write (see "Work distribution")
                 const uint32_t* cnt = p.sync + 2 + (u - work.u_base);
-                const uint32_t want = c * 4 * CG;
+                const uint32_t want = c * GM_EPI_WARPS * CG;
                 const long long t0 = clock64();
                 while (ptx::ld_acquire_gpu(cnt) < want) {
                     if (clock64() - t0 > (20ll << 30)) __trap();  // ~10 s: never in a correct run
@@ -418,7 +421,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 const uint64_t row = (uint64_t)((mt * rsub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
                 const bool row_ok = row < p.rows;
                 const uint32_t tacc = tmem_base + ((quarter * 32) << 16) + as * acc_cols + m * NL * p.bn;
-                for (uint32_t g0 = 0; g0 < p.qt / 4; g0 += kPf) {
+                for (uint32_t g0 = half * kPf; g0 < p.qt / 4; g0 += 2 * kPf) {
                     uint32_t old[4 * kPf];
                     if (need_old) {
 #pragma unroll
