@@ -516,7 +516,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             if (u >= work.u_base) __threadfence();  // this lane's answer words, before the arrival below
             __syncwarp();
             if (lane == 0) {
-                if constexpr (CG == 2) ptx::mbar_arrive_cluster(&tmem_empty[as], 0);
+                if constexpr (CG == 2) ptx::mbar_arrive_cluster_relaxed(&tmem_empty[as], 0);
                 else ptx::mbar_arrive(&tmem_empty[as]);
                 // units of the leftover round may be shared with another group: count this warp in
                 if (u >= work.u_base) ptx::red_release_gpu_add(p.sync + 2 + (u - work.u_base), 1u);

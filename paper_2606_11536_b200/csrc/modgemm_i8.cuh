@@ -469,7 +469,7 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) {
-                    if constexpr (CG == 2) ptx::mbar_arrive_cluster(&tmem_empty[as], 0);
+                    if constexpr (CG == 2) ptx::mbar_arrive_cluster_relaxed(&tmem_empty[as], 0);
                     else ptx::mbar_arrive(&tmem_empty[as]);
                 }
             }

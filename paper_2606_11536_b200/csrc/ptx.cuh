@@ -92,6 +92,14 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t rank
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(mapa(smem_u32(bar), rank))
                  : "memory");
 }
+// Same without memory-ordering semantics: for arrivals that only say "my tcgen05.ld reads of this accumulator stage
+// are complete" (they are, once tcgen05.wait::ld has returned: the data sits in registers), where the release form's
+// GPU-scope membar would also wait for every global store the warp has in flight -- over PCIe when the answer goes to
+// mapped host memory.
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint64_t* bar, uint32_t rank) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(mapa(smem_u32(bar), rank))
+                 : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
