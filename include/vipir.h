@@ -200,12 +200,13 @@ int vipir_dbmul(vipir_plan *plan, const void *d_db, const uint32_t *d_query, uin
  * pointers with the d_query / d_answer layouts; d_db: DEVICE pointer.  The first call allocates device
  * staging, a copy stream and events, all owned by the plan.
  *   Pinned memory (cudaHostAlloc / cudaHostRegister) makes the copies asynchronous.  When h_answer is
- * pinned and device-mapped, the kernels store the finished answer words into it directly (plain 128-byte
- * stores over PCIe while the scan runs) and no device-to-host copy is made.
+ * pinned and device-mapped, the kernels write the finished answer words into it themselves while the scan
+ * runs (batch 1: the scan's own stores; tensor-core regimes: two warps of every CTA copy each finished tile
+ * from device staging) and no device-to-host copy is made.
  *   Tensor-core regimes: the call is pipelined over K slices (PAPER.md:245-249's K chunks, grouped): the
  * copy stream brings slice i's columns of every query vector and splits them into limbs while the caller's
- * stream scans slice i-1; every slice adds to the running sums (device staging), the last one writes the
- * result.  Same answer, bit for bit, as vipir_dbmul.  vipir_tuning.host_staged = 1 selects the plain form
+ * stream scans slice i-1; every slice adds to the running sums (device staging).  Same answer, bit for bit,
+ * as vipir_dbmul.  vipir_tuning.host_staged = 1 selects the plain form
  * (one copy in, vipir_dbmul, one copy out).
  */
 int vipir_dbmul_host(vipir_plan *plan, const void *d_db, const uint32_t *h_query, uint32_t *h_answer,

@@ -16,7 +16,7 @@
 //            CTA, N <= 256 per instruction, K = 32 bytes), accumulators in TMEM; the limb
 //            planes are laid out so that the LC limb sums of one query are LC adjacent
 //            accumulator columns;
-//   warp 2   TMEM allocator;
+//   warp 2   TMEM allocator; warps 2-3 copy finished units to final_out when the host call wants the result there;
 //   warps 4-11 epilogue (two per TMEM lane quarter, taking alternate batches of 32 query vectors):
 //            tcgen05.ld the accumulators of their lane quarter, recombine limbs
 //            with shifts (wrap mod 2^32) or in u64 + Barrett (prime moduli), and store /
@@ -99,8 +99,8 @@ struct GemmParams {
     uint64_t barrett[GM_MAX_MODULI];  // floor(2^64 / p)
     uint32_t acc_in;         // 1: `answer` already holds the sum over the K range before k_begin (an earlier launch's)
     uint32_t* answer;        // [nq][rows]: running sums between K chunks, and the result unless final_out differs
-    uint32_t* final_out;     // where the LAST chunk of this launch writes (== answer, or e.g. mapped host memory:
-                             // plain stores only, the running sum is read from `answer`)
+    uint32_t* final_out;     // == answer, or where the result is wanted besides (mapped host memory): warps 2-3 of every
+                             // CTA copy a unit's words there once its LAST chunk of this launch is in `answer`
 };
 
 // K-major, 128B-swizzled shared-memory operand descriptor (8-row x 128-byte atoms, 1024 B apart)
@@ -203,9 +203,13 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     uint64_t* empty = full + p.stages;
     uint64_t* tmem_full = empty + p.stages;   // [2]
     uint64_t* tmem_empty = tmem_full + 2;     // [2]
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    uint64_t* copy_full = tmem_empty + 2;     // [2]  finished units handed to the copier warps (final_out != answer)
+    uint64_t* copy_empty = copy_full + 2;     // [2]
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(copy_empty + 2);
     uint32_t* ticket_ptr = tmem_ptr + 1;
     uint32_t* last_ptr = tmem_ptr + 2;
+    uint32_t* copy_unit = tmem_ptr + 3;       // [2]
+    const bool copier = p.final_out != p.answer;
 
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
@@ -233,6 +237,8 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         for (uint32_t a = 0; a < 2; ++a) {
             ptx::mbar_init(&tmem_full[a], 1);
             ptx::mbar_init(&tmem_empty[a], GM_EPI_WARPS * CG);  // one arrival per epilogue warp of every CTA
+            ptx::mbar_init(&copy_full[a], GM_EPI_WARPS);        // this CTA's epilogue warps
+            ptx::mbar_init(&copy_empty[a], 2);                  // this CTA's two copier warps
         }
         ptx::fence_barrier_init();
     }
@@ -381,11 +387,55 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 }
             });
         }
-    } else if (warp >= 4) {
+    } else if (copier && warp < 4) {
+        // ===== warps 2-3, only when the result is wanted in final_out (the host call's mapped answer buffer): move every
+        // finished unit's words of this CTA from `answer` (device memory, just written: L2) to final_out.  The epilogue
+        // warps cannot store there themselves without holding the accumulators for as long as the host link takes
+        // (one unit's 64 KB per CTA is ~185 us of a saturated link, the unit's products ~210 us): measured 0.4-0.5 ms per
+        // configs[3] call.  Here the stores of unit u run beside the products of unit u + 1. =====
+        const uint32_t cw = warp - 2;
+        const bool vec = (p.rows % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.answer) | reinterpret_cast<uintptr_t>(p.final_out)) & 15) == 0;
+        uint32_t n_final = 0;
+        for_each_item(work, [&](uint32_t, uint32_t c, bool) {
+            if (c + 1 != p.n_chunks) return;
+            const uint32_t slot = n_final & 1, ph = (n_final >> 1) & 1;
+            ++n_final;
+            ptx::mbar_wait(&copy_full[slot], ph);
+            const uint32_t u = *reinterpret_cast<volatile uint32_t*>(&copy_unit[slot]);
+            const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
+            const uint32_t q_lo = nt * p.qt, q_hi = min(p.nq, q_lo + p.qt);
+            for (uint32_t m = 0; m < rsub; ++m) {
+                const uint64_t row0 = (uint64_t)((mt * rsub + m) * CG + rank) * GM_BM;
+                if (row0 >= p.rows) break;
+                const uint32_t n_rows = (uint32_t)min((uint64_t)GM_BM, p.rows - row0);
+                if (vec) {  // a warp moves one query vector's 128 rows (512 bytes) per step, eight steps in flight
+                    constexpr uint32_t kU = 8;
+                    for (uint32_t q0 = q_lo + cw * kU; q0 < q_hi; q0 += 2 * kU) {
+                        uint4 v[kU];
+#pragma unroll
+                        for (uint32_t j = 0; j < kU; ++j)
+                            if (q0 + j < q_hi && lane * 4 < n_rows)
+                                v[j] = __ldcg(reinterpret_cast<const uint4*>(p.answer + (uint64_t)(q0 + j) * p.rows + row0) + lane);
+#pragma unroll
+                        for (uint32_t j = 0; j < kU; ++j)
+                            if (q0 + j < q_hi && lane * 4 < n_rows)
+                                reinterpret_cast<uint4*>(p.final_out + (uint64_t)(q0 + j) * p.rows + row0)[lane] = v[j];
+                    }
+                } else {
+                    for (uint32_t q = q_lo + cw; q < q_hi; q += 2)
+                        for (uint32_t r = lane; r < n_rows; r += 32)
+                            p.final_out[(uint64_t)q * p.rows + row0 + r] = __ldcg(p.answer + (uint64_t)q * p.rows + row0 + r);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&copy_empty[slot]);
+        });
+    }
+    if (warp >= 4) {
         // ===== epilogue warps: lane quarter = warp % 4; the two warps of a quarter take alternate batches of kPf steps =====
         const uint32_t quarter = warp & 3;
         const uint32_t half = (warp - 4) >> 2;
-        uint32_t acc_it = 0;
+        uint32_t acc_it = 0, n_final = 0;
         for_each_item(work, [&](uint32_t u, uint32_t c, bool must_wait) {
             const uint32_t mt = u / p.n_tiles, nt = u % p.n_tiles;
             const uint32_t as = acc_it % p.acc_stages;
@@ -411,12 +461,11 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             constexpr uint32_t kPf = 8;
             const bool first = c == 0 && !p.acc_in;   // nothing accumulated yet: plain store
             const bool last = c + 1 == p.n_chunks;
-            // the last chunk writes the result to final_out; when that is not the running-sum buffer (the
-            // host call's mapped answer) it needs the running sum back as well, and stores instead of adding
-            const bool redirect = last && p.final_out != p.answer;
             const bool ms_final = !PRIME && p.ms_bits != 0 && last;
-            const bool need_old = !first && (PRIME || ms_final || redirect);
-            uint32_t* const obase = last ? p.final_out : p.answer;
+            const bool need_old = !first && (PRIME || ms_final);
+            // every chunk lands in `answer`; when the result is wanted elsewhere (final_out: the host call's mapped
+            // answer) the CTA's copier warps move a unit there once its last chunk is in (below)
+            uint32_t* const obase = p.answer;
             for (uint32_t m = 0; m < rsub; ++m) {
                 const uint64_t row = (uint64_t)((mt * rsub + m) * CG + rank) * GM_BM + quarter * 32 + lane;
                 const bool row_ok = row < p.rows;
@@ -500,8 +549,6 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                     *dst = modswitch_word(val, p.ms_bits);
                                 } else if (first) {
                                     *dst = val;
-                                } else if (redirect) {
-                                    *dst = val + old[gg * 4 + i];
                                 } else {
                                     asm volatile("red.global.add.u32 [%0], %1;" ::"l"(dst), "r"(val) : "memory");
                                 }
@@ -513,14 +560,28 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
             // accumulator stage drained
             ptx::tc_fence_before();
-            if (u >= work.u_base) __threadfence();  // this lane's answer words, before the arrival below
             __syncwarp();
             if (lane == 0) {
                 if constexpr (CG == 2) ptx::mbar_arrive_cluster_relaxed(&tmem_empty[as], 0);
                 else ptx::mbar_arrive(&tmem_empty[as]);
-                // units of the leftover round may be shared with another group: count this warp in
-                if (u >= work.u_base) ptx::red_release_gpu_add(p.sync + 2 + (u - work.u_base), 1u);
             }
+            // this lane's answer words, before the arrivals below: for the group that continues a leftover unit,
+            // and for the copier warps that move a finished unit to final_out
+            if (u >= work.u_base || (copier && last)) __threadfence();
+            __syncwarp();
+            if (copier && last) {
+                // hand the finished unit to this CTA's copier warps: a ring of two entries, the n-th finished unit of
+                // this CTA in entry n % 2 (the copiers walk the same work items and count the same way)
+                const uint32_t slot = n_final & 1, ph = (n_final >> 1) & 1;
+                ++n_final;
+                ptx::mbar_wait(&copy_empty[slot], ph ^ 1);
+                if (lane == 0) {
+                    if (warp == 4) *reinterpret_cast<volatile uint32_t*>(&copy_unit[slot]) = u;
+                    ptx::mbar_arrive(&copy_full[slot]);  // release: the unit id (warp 4) and the fence above
+                }
+            }
+            // units of the leftover round may be shared with another group: count this warp in
+            if (lane == 0 && u >= work.u_base) ptx::red_release_gpu_add(p.sync + 2 + (u - work.u_base), 1u);
         });
     }
 

@@ -232,7 +232,7 @@ int plan_gemm(vipir_plan* p, int cg) {
         const uint64_t rows_unit = 128ull * cg * (cand / nl);
         const uint64_t units = (p->rows + rows_unit - 1) / rows_unit * g.n_tiles;
         const uint32_t atom = cand * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
-        if (2 * cand * bn <= 512 && 3 * atom <= kMaxSmem - 1280 && units * g.n_chunks >= 2ull * max_groups) {
+        if (2 * cand * bn <= 512 && 3 * atom <= kMaxSmem - 1408 && units * g.n_chunks >= 2ull * max_groups) {
             msub = cand;
             break;
         }
@@ -245,7 +245,7 @@ int plan_gemm(vipir_plan* p, int cg) {
     const uint64_t rows_unit = 128ull * cg * (msub / nl);
     g.m_tiles = (uint32_t)((p->rows + rows_unit - 1) / rows_unit);
     g.atom_bytes = msub * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
-    const uint32_t overhead = 1024 + 256;  // alignment slack + barriers
+    const uint32_t overhead = 1024 + 384;  // alignment slack + barriers (ring, accumulator, copier) and the words behind them
     // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes")
     // measured on B200 (profiles/r01_tuning.md): several k-atoms per stage (longer contiguous DB
     // runs per row, fewer barrier round trips) beat deeper rings of single atoms; keep >= 3 stages
@@ -613,8 +613,9 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
         cudaGetLastError();
         return VIPIR_ERR_ALLOC;
     }
-    // with pinned, device-mapped host memory the kernels store the answer into it directly: their plain 128-byte
-    // stores go over PCIe while the scan runs, and the device-to-host copy after it disappears
+    // with pinned, device-mapped host memory the kernels write the answer into it themselves while the scan runs
+    // (batch 1: the scan's own 128-byte stores; tensor regimes: copier warps, gemm_i8_tcgen05.cuh), and the
+    // device-to-host copy after it disappears
     uint32_t* d_direct = p->tune.host_staged ? nullptr : mapped_device_pointer(h_answer);
     const bool mma = p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM;
 
@@ -628,7 +629,7 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     uint32_t bounds[kMaxHostSlices + 1];
     const uint32_t S = (mma && !p->tune.host_staged) ? host_slices(p, qbytes, bounds) : 1u;
     // the running sums between K chunks / slices are read back by the kernels: they stay in device memory
-    const bool need_stage = !d_direct || S > 1 || p->gm.n_chunks > 1 || !mma;
+    const bool need_stage = true;  // the kernels accumulate in device memory; the mapped host buffer only receives finished units
     if (need_stage && !p->d_a_stage && cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
         cudaGetLastError();
         return VIPIR_ERR_ALLOC;
@@ -643,8 +644,8 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     }
     // ---- tensor-core regimes: copy / split / scan pipelined over K slices ----
     // copy stream: H2D of slice i's columns of every query vector (a strided copy), its split;  caller's stream:
-    // the scan of slice i, which adds to the running sums of the slices before it.  The last slice's last chunk
-    // writes the finished words to the host buffer (directly when it is mapped).
+    // the scan of slice i, which adds to the running sums of the slices before it (device staging).  In the last
+    // slice every CTA copies its finished units to the host buffer when that is mapped (final_out).
     if (!p->copy_stream) {  // all of them or none: a later call must not find a stream without its events
         cudaStream_t cs = nullptr;
         cudaEvent_t ev[kMaxHostSlices + 1] = {};
