@@ -36,8 +36,10 @@
  * owns one limb-plane workspace, one set of staging buffers and cached tensor maps.  (Per-call
  * values -- the answer pointer, the modulus-switch and signedness flags in effect -- are passed
  * to the kernels by value; the planned parameters are never rewritten by a call.)  A server
- * that overlaps requests makes one plan per stream.  All kernels are sm_100a; there is no
- * fallback of any kind.
+ * that overlaps requests makes one plan per stream.  After one call outside the capture (which
+ * sets kernel attributes and encodes the tensor maps for these buffers) a vipir_dbmul call can be
+ * captured into a CUDA graph and replayed: the kernels reset their own work counters.  All
+ * kernels are sm_100a; there is no fallback of any kind.
  *
  * Errors: every entry point returns a vipir_status (0 = OK) and never throws or aborts.
  */

@@ -565,6 +565,35 @@ def test_two_plans_two_threads_two_streams():
     assert not errors, errors
 
 
+@pytest.mark.parametrize("regime,batch,moduli", [(G, 1, None), (M1, 8, None), (M2, 40, PRIMES)])
+def test_device_call_is_cuda_graph_capturable(regime, batch, moduli):
+    """vipir_dbmul only enqueues kernels (no allocation, no synchronisation, work counters reset by the kernel itself), so a
+    call can be captured into a CUDA graph and replayed with new query contents in the same buffers."""
+    import torch
+    ensure_built()
+    rows, cols = 700, 33024 if regime != G else 2080   # two K chunks in the tensor regimes: units shared between groups
+    D = inputs.db_rows(77, rows, cols, 8)
+    d_db = torch.from_numpy(D).cuda()
+    T = 1 if moduli is None else len(moduli)
+    d_q = torch.zeros((T, batch, cols), dtype=torch.int32, device="cuda")
+    d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")
+    with vipir.Plan(rows, cols, batch, 8, moduli, regime) as plan:
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            plan(d_db, d_q, d_a)            # first call outside the capture: sets the kernels' attributes, encodes the maps
+            side.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                plan(d_db, d_q, d_a)
+        for seed in (1, 2, 3):
+            Q = inputs.query(300 + seed, cols, batch, moduli)
+            d_q.copy_(torch.from_numpy(Q.view(np.int32)))
+            d_a.fill_(-1)
+            graph.replay()
+            torch.cuda.synchronize()
+            assert_same(d_a.cpu().numpy().view(np.uint32), oracle.dbmul(D, Q, moduli, nthreads=NT))
+
+
 def test_misaligned_pointers_are_rejected():
     import torch
     ensure_built()
