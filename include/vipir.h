@@ -338,7 +338,7 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan **out, uint32_t T, uint64
  * PAPER.md:222).  Must run before the first vipir_modgemm / vipir_modgemm_products. */
 int vipir_modgemm_set_h(vipir_modgemm_plan *plan, const uint32_t *d_H, void *cuda_stream);
 
-/* ONLINE step: enqueue Out = H*C + (0|G) mod q_t.  From 32 columns up (and K % 4 == 0: the paper's n = 1280) ONE
+/* ONLINE step: enqueue Out = H*C + (0|G) mod q_t.  From 16 columns up (and K % 4 == 0: the paper's n = 1280) ONE
  * kernel: the tensor-core kernel reads the raw words of C by TMA and splits them into limbs in shared memory (the
  * paper fuses its prmt decomposition into the GEMM kernel as well); below that, where it measures
  * faster, the C limb splitter followed by the tensor-core kernel (vipir_modgemm_info_t.launches says which;

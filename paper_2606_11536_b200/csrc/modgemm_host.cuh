@@ -113,18 +113,23 @@ int plan_modgemm(vipir_modgemm_plan* p) {
     p->mg_fused = g;
     if (p->fused) {
         vipir::ModGemmParams& f = p->mg_fused;
-        f.b_stages = p->tune.b_stages ? p->tune.b_stages : 2;
         // every CTA brings the raw words of the whole tile, per k-atom four 32-word boxes of ct rows (a multiple of
-        // 1 KiB, so every box starts on a swizzle atom).  The raw words of k-atom a are requested when the slot of
-        // atom a - r_stages has been converted; measured at B = 32 (ct = 64, 32 KiB a slot), what the ring takes from
-        // the H ring costs more than a third slot gains (two slots + 8 H boxes 4.95 ms, three + 6: 5.20 ms), so:
-        // the deepest ring that leaves the H ring eight boxes (two k-atoms), at least two slots
+        // 1 KiB, so every box starts on a swizzle atom).  The raw tiles are requested r_stages - 1 k-atoms ahead of
+        // the H boxes (modgemm_i8.cuh), which makes the H ring's depth uncritical (64 columns: 4.94 / 4.95 / 4.92 ms
+        // with 4 / 6 / 8 H boxes); what pays is the depth of the converted-operand ring, which decouples the
+        // converters from the MMA issuer: at 64 columns b = 2 / 3 with r = 2: 4.95 / 4.59 ms, r = b = 3 (5 H boxes)
+        // 4.50 ms, b = 4 no better; at 32 columns r = b = 4: 3.40 against 3.48 ms.  So: four and four slots when
+        // eight H boxes remain, else three and three with at least five, else three and two, else two and two.
         f.r_stage_bytes = 4 * ct * 128;
-        auto fits = [&](uint32_t r, uint32_t a) {
-            return overhead + f.b_stages * f.b_stage_bytes + r * f.r_stage_bytes + a * vipir::MG_A_BYTES <= kMaxSmem;
+        auto fits = [&](uint32_t r, uint32_t b, uint32_t a) {
+            return overhead + b * f.b_stage_bytes + r * f.r_stage_bytes + a * vipir::MG_A_BYTES <= kMaxSmem;
         };
-        f.r_stages = fits(4, 8) ? 4u : fits(3, 8) ? 3u : 2u;
-        if (const uint32_t r_force = p->tune.r_stages) f.r_stages = r_force;
+        if (fits(4, 4, 8)) f.r_stages = 4, f.b_stages = 4;
+        else if (fits(3, 3, 5)) f.r_stages = 3, f.b_stages = 3;
+        else if (fits(2, 3, 6)) f.r_stages = 2, f.b_stages = 3;
+        else f.r_stages = 2, f.b_stages = 2;
+        if (p->tune.b_stages) f.b_stages = p->tune.b_stages;
+        if (p->tune.r_stages) f.r_stages = p->tune.r_stages;
         const uint32_t fixed = overhead + f.b_stages * f.b_stage_bytes + f.r_stages * f.r_stage_bytes;
         if (fixed + 4 * vipir::MG_A_BYTES > kMaxSmem) return VIPIR_ERR_UNSUPPORTED;
         f.a_stages = (kMaxSmem - fixed) / vipir::MG_A_BYTES;
@@ -255,13 +260,14 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
     // One kernel (C split into limbs inside the products kernel) or two (a splitter pre-pass writes C's limb planes).
     // The raw-C tensor map needs 16-byte row strides: K % 4 == 0 (the paper's n = 1280).  Measured at the paper's shape
     // (sustained, same run): 64 columns 4.95 against 5.6 ms, 16 columns 3.01 against 2.93 ms, 2 columns 2.51 against
-    // 2.42 ms -- the pre-pass costs 2 * 4 bytes per word of C, the fused form a longer dependency chain per k-atom:
-    // fused from 32 columns up.
+    // 2.42 ms -- the pre-pass costs 2 * 4 bytes per word of C, the fused form a longer dependency chain per k-atom.
+    // With the raw tiles requested ahead and deeper operand rings (plan_modgemm): 64 columns 4.50 against 5.4 ms,
+    // 32 columns 3.40 against 3.64, 16 columns 2.91 against 2.94, 2 columns 2.48 against 2.42: fused from 16 columns up.
     if (p->tune.c_split == 2 && K % 4 != 0) {
         delete p;
         return VIPIR_ERR_UNSUPPORTED;
     }
-    p->fused = p->tune.c_split ? p->tune.c_split == 2 : (K % 4 == 0 && ncols >= 32);
+    p->fused = p->tune.c_split ? p->tune.c_split == 2 : (K % 4 == 0 && ncols >= 16);
     p->hp_bytes = p->P * M * 4ull * p->Kp;
     p->cp_bytes = p->P * 4ull * ncols * p->Kp;
     // the C limb planes are only needed by the two-kernel form: allocated here when that is the plan's form,

@@ -215,26 +215,37 @@ modgemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             uint32_t sa = 0, pa = 0, sb = 0, pb = 0;
             // H is streamed once when there is a single N tile; sibling N tiles re-read it from L2
             const uint64_t hintA = (p.n_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+            // FUSED: the raw words of the C tiles run AHEAD of the H boxes by r_stages - 1 k-atoms (a cursor of their
+            // own, across unit boundaries): they have the longer way to the tensor core (load, conversion, hand-over),
+            // and requested in step with the H boxes of their k-atom they arrive late whenever the H ring is short
+            // (measured at 64 columns: 5.36 / 5.07 / 4.86 ms with 4 / 6 / 8 H boxes before this)
+            uint32_t ur = unit0, ar = 0;
+            auto raw_next = [&]() {
+                if (ur >= n_units) return;
+                const uint32_t prob = ur / tiles_per_problem, nt = (ur % tiles_per_problem) % p.n_tiles;
+                ptx::mbar_wait(&emptyR[sb], pb ^ 1);
+                __syncwarp();
+                uint8_t* dR = sR_ring + (size_t)sb * p.r_stage_bytes;
+                if (ptx::elect_one()) {
+                    ptx::mbar_arrive_expect_tx(&fullR[sb], p.r_stage_bytes);
+#pragma unroll
+                    for (uint32_t kb = 0; kb < 4; ++kb)  // every CTA its own copy: four 32-word k-blocks
+                        ptx::tma_load_3d(dR + kb * (p.r_stage_bytes / 4), &tmB, &fullR[sb], (int32_t)(ar * MG_BK + kb * 32),
+                                         (int32_t)(nt * p.ct), (int32_t)prob, ptx::kEvictNormal);
+                }
+                __syncwarp();
+                if (++sb == p.r_stages) { sb = 0; pb ^= 1; }
+                if (++ar == p.atoms) { ar = 0; ur += unit_stride; }
+            };
+            if constexpr (FUSED)
+                for (uint32_t i = 0; i + 1 < p.r_stages; ++i) raw_next();
             for (uint32_t u = unit0; u < n_units; u += unit_stride) {
                 const uint32_t prob = u / tiles_per_problem, rem = u % tiles_per_problem;
                 const uint32_t mt = rem / p.n_tiles, nt = rem % p.n_tiles;
                 const int32_t row0 = (int32_t)((mt * CG + rank) * MG_BM);
                 for (uint32_t a = 0; a < p.atoms; ++a) {
                     if constexpr (FUSED) {
-                        // the raw words of the C tile (every CTA its own copy): four 32-word k-blocks
-                        ptx::mbar_wait(&emptyR[sb], pb ^ 1);
-                        __syncwarp();
-                        uint8_t* dR = sR_ring + (size_t)sb * p.r_stage_bytes;
-                        if (ptx::elect_one()) {
-                            ptx::mbar_arrive_expect_tx(&fullR[sb], p.r_stage_bytes);
-#pragma unroll
-                            for (uint32_t kb = 0; kb < 4; ++kb)
-                                ptx::tma_load_3d(dR + kb * (p.r_stage_bytes / 4), &tmB, &fullR[sb],
-                                                 (int32_t)(a * MG_BK + kb * 32), (int32_t)(nt * p.ct), (int32_t)prob,
-                                                 ptx::kEvictNormal);
-                        }
-                        __syncwarp();
-                        if (++sb == p.r_stages) { sb = 0; pb ^= 1; }
+                        raw_next();
                     } else {
                     ptx::mbar_wait(&emptyB[sb], pb ^ 1);
                     __syncwarp();

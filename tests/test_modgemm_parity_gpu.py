@@ -39,7 +39,7 @@ def run_modgemm(H, C, G, moduli, cg=0, ct=0, return_info=False, via_parts=False)
     fusable = K % 4 == 0
     with vipir.ModGemmPlan(T, NC, M, K, ncols, gcols, moduli, tuning=tuning) as plan:
         plan.set_h(d_H)
-        assert plan.info["fused_split"] == (1 if fusable and ncols >= 32 else 0)  # the planner's rule (include/vipir.h)
+        assert plan.info["fused_split"] == (1 if fusable and ncols >= 16 else 0)  # the planner's rule (include/vipir.h)
         assert plan.info["launches"] == 2 - plan.info["fused_split"]
         if via_parts:
             vipir.modgemm_split_c(plan.handle, d_C)
