@@ -298,7 +298,8 @@ typedef struct {
     uint32_t mma_n;         /* N of one tcgen05.mma = 4 * ct */
     uint32_t m_tiles, n_tiles; /* per problem */
     uint32_t n_chunks;      /* K chunks of <= 8192 (int32 accumulation bound 4*255^2*K < 2^31) */
-    uint32_t a_stages, b_stages, acc_stages;
+    uint32_t a_stages, b_stages, acc_stages; /* ring depths: H boxes, converted C operand slots; accumulator stages */
+    uint32_t r_stages;      /* one-kernel form: ring depth of the raw C tiles (0 otherwise) */
     uint32_t smem_bytes, grid;
     uint32_t launches;      /* kernels enqueued per vipir_modgemm call: 1 when the C limb split is fused in */
     uint32_t fused_split;   /* 1: vipir_modgemm splits C inside the products kernel, no C limb planes */

@@ -362,6 +362,7 @@ int vipir_modgemm_info(const vipir_modgemm_plan* p, vipir_modgemm_info_t* o) {
     o->a_stages = g.a_stages;
     o->b_stages = g.b_stages;
     o->acc_stages = g.acc_stages;
+    o->r_stages = p->fused ? g.r_stages : 0;
     o->smem_bytes = p->fused ? p->smem_bytes_fused : p->smem_bytes;
     o->grid = p->grid;
     o->launches = p->fused ? 1 : 2;

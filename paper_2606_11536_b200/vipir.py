@@ -78,7 +78,8 @@ class ModGemmInfo(ctypes.Structure):
         ("problems", ctypes.c_uint64), ("k_padded", ctypes.c_uint32), ("cta_group", ctypes.c_uint32),
         ("tile_cols", ctypes.c_uint32), ("mma_n", ctypes.c_uint32), ("m_tiles", ctypes.c_uint32),
         ("n_tiles", ctypes.c_uint32), ("n_chunks", ctypes.c_uint32), ("a_stages", ctypes.c_uint32),
-        ("b_stages", ctypes.c_uint32), ("acc_stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
+        ("b_stages", ctypes.c_uint32), ("acc_stages", ctypes.c_uint32), ("r_stages", ctypes.c_uint32),
+        ("smem_bytes", ctypes.c_uint32),
         ("grid", ctypes.c_uint32), ("launches", ctypes.c_uint32), ("fused_split", ctypes.c_uint32),
         ("h_limb_bytes", ctypes.c_uint64), ("c_limb_bytes", ctypes.c_uint64),
     ]

@@ -154,6 +154,21 @@ def test_modgemm_identity_and_probe():
             assert np.array_equal(got[0, c, j], (np.roll(pi, c) + 1 + j * K).astype(np.uint32))
 
 
+def test_modgemm_planner_choices_at_the_paper_shape():
+    """Form and ring depths the planner takes at the paper's per-problem shape 256 x 2B x 1280 (include/vipir.h,
+    DESIGN.md section 12): two kernels below 16 columns; one kernel from there on, with the deepest raw / operand rings
+    that leave the H ring its minimum."""
+    ensure_built()
+    for B, want in ((1, dict(fused_split=0, launches=2, cta_group=1)),
+                    (8, dict(fused_split=1, launches=1, cta_group=2, tile_cols=16, r_stages=4, b_stages=4)),
+                    (16, dict(fused_split=1, tile_cols=32, r_stages=4, b_stages=4, acc_stages=2)),
+                    (32, dict(fused_split=1, tile_cols=64, r_stages=3, b_stages=3, a_stages=5, acc_stages=1))):
+        with vipir.ModGemmPlan(3, 8, 256, 1280, 2 * B, B, P29) as plan:
+            got = {k: plan.info[k] for k in want}
+            assert got == want, (B, plan.info)
+            assert plan.info["a_stages"] >= 5 and plan.info["smem_bytes"] <= 232448
+
+
 def test_modgemm_split_kernels_layout():
     # the limb re-layouts on their own, against their stated layouts (include/vipir.h)
     import torch
