@@ -251,6 +251,50 @@ int vipir_plan_info(const vipir_plan *plan, vipir_info *out);
 /* Free the plan and its workspace.  vipir_destroy(NULL) is a no-op. */
 void vipir_destroy(vipir_plan *plan);
 
+/*
+ * The batched product for callers that cannot allocate device memory: no plan, no cudaMalloc, no cudaFree, no
+ * library routine that allocates -- the call only encodes tensor maps on the host and enqueues a memset and two
+ * kernels on `cuda_stream`.  Same definition and the same answer, bit for bit, as vipir_dbmul
+ * (answer = D * Q mod q, by the limb decomposition of PAPER.md:245-249).
+ *
+ * Who needs this.  A PIR server keeps the whole database resident in GPU DRAM, so a deployment
+ * typically hands all device memory out once at start-up -- to the database and to one arena that some other
+ * runtime owns -- and a later cudaMalloc from inside a library either fails or eats into that arena behind its
+ * owner's back.  Request handlers on a latency budget are in the same position for another reason: cudaMalloc
+ * and cudaFree may synchronise the whole device, which stalls every other request's stream while they run.
+ * Such callers cannot build a vipir_plan (it allocates the query limb planes and a few counters); they call this.
+ *
+ * How it works.  The tensor-core kernel's scratch (the limb planes written by the query splitter, and its
+ * work-distribution counters) lives in a fixed array inside the library image, 4 KiB + VIPIR_STATIC_SCRATCH_BYTES
+ * (8 MiB) long.  Every GPU on which the library's kernels are loaded holds that array until the process exits,
+ * whether or not this entry point is ever used.  The caller passes inputs and outputs only:
+ *   rows, cols, batch, db_bits, mod   the shape, as for vipir_dbmul_plan (database row-major; q = 2^32 or primes)
+ *   d_db, d_query, d_answer           DEVICE pointers with vipir_dbmul's layouts, alignment and ownership rules
+ * Always the tensor-core kernel (1-SM tiles or CTA pairs by AUTO's rule), also for batch 1, where a plan would
+ * pick the faster GEMV regime.
+ *
+ * Limit.  The limb planes must fit: T * batch * LC * cols * db_bits/8 <= VIPIR_STATIC_SCRATCH_BYTES
+ * (LC = 4; 5 for a u16 database with prime moduli).  For a u8 database that is 256 query vectors at cols = 8192,
+ * 16 at cols = 131072.  Anything larger returns VIPIR_ERR_UNSUPPORTED before any device work, and
+ * vipir_last_cuda_error() then holds a sentence with the bytes needed and the bytes available.
+ *
+ * First call on each device: looks up the array's address on that device (the current device must be the one the
+ * pointers belong to) and sets the kernels' shared-memory attribute.  Make that first call during start-up, before
+ * any stream capture begins.  Later calls skip the set-up.
+ *
+ * Shared state.  All calls on one GPU -- from any thread, on any stream -- use the same array, and it keeps the
+ * previous call's contents.  The call clears the counters itself (on `cuda_stream`, ahead of the kernels) and the
+ * splitter overwrites every plane byte the scan reads, so a stale array is harmless; but two calls whose GPU work
+ * overlaps in time race on it and both answers are undefined.  Issue them on one stream, or order the streams with
+ * events.  The call does not wait for the GPU: d_answer is valid once `cuda_stream` has run it.
+ *
+ * Errors: INVALID_ARG and UNSUPPORTED as for vipir_dbmul_plan / vipir_dbmul, UNSUPPORTED for the size limit above or
+ * a device ordinal >= 64, ARCH, CUDA.  Never ALLOC.
+ */
+#define VIPIR_STATIC_SCRATCH_BYTES (8u << 20)
+int vipir_dbmul_static(uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits, const vipir_modulus_spec *mod,
+                       const void *d_db, const uint32_t *d_query, uint32_t *d_answer, void *cuda_stream);
+
 /* Static string for a status code. */
 const char *vipir_status_str(int status);
 

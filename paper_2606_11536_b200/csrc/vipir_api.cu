@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include <cuda.h>
@@ -783,6 +784,126 @@ void vipir_destroy(vipir_plan* p) {
 }
 
 }  // extern "C"
+
+// ---- vipir_dbmul_static: the tensor-core product for callers that must not allocate (include/vipir.h) ----------
+//
+// The tensor-core kernel needs two pieces of global memory besides its inputs and outputs: the query limb planes
+// the splitter writes for it, and a few work-distribution counters.  A plan gets them from cudaMalloc.  This
+// entry point keeps them in an array that is part of the library image instead, so the call itself never asks
+// the driver for memory.  Layout: [0, 4096) the counters, [4096, 4096 + VIPIR_STATIC_SCRATCH_BYTES) the planes.
+namespace {
+
+constexpr uint32_t kStaticSyncBytes = 4096;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticSyncBytes + VIPIR_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` is only a handle for the runtime, not an address a kernel can use.  The real
+// device address differs per GPU, so it is looked up once per device (with that device current) and remembered.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned char* g_static_ptr[kStaticMaxDevices] = {};
+int g_static_sms[kStaticMaxDevices] = {};
+
+int static_scratch_setup(int dev, unsigned char** ptr, int* sms) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        int major = 0, minor = 0, n = 0;
+        CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        CK(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
+        CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
+        if (major != 10 || minor != 0) return VIPIR_ERR_ARCH;
+        void* a = nullptr;
+        CK(cudaGetSymbolAddress(&a, g_static_scratch));
+        if (!a) {
+            snprintf(g_cuda_err, sizeof g_cuda_err, "cudaGetSymbolAddress returned a null address");
+            return VIPIR_ERR_CUDA;
+        }
+        g_static_sms[dev] = n;
+        g_static_ptr[dev] = static_cast<unsigned char*>(a);
+    }
+    *ptr = g_static_ptr[dev];
+    *sms = g_static_sms[dev];
+    return VIPIR_OK;
+}
+
+}  // namespace
+
+extern "C" int vipir_dbmul_static(uint64_t rows, uint64_t cols, uint32_t batch, uint32_t db_bits,
+                                  const vipir_modulus_spec* mod, const void* d_db, const uint32_t* d_query,
+                                  uint32_t* d_answer, void* cuda_stream) {
+    g_cuda_err[0] = 0;
+    // ---- the argument rules of vipir_dbmul_plan and vipir_dbmul; none of them needs a device ----
+    if (!d_db || !d_query || !d_answer) return VIPIR_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
+        (reinterpret_cast<uintptr_t>(d_answer) & 3))
+        return VIPIR_ERR_INVALID_ARG;
+    if (rows == 0 || cols == 0 || batch == 0) return VIPIR_ERR_INVALID_ARG;
+    if (db_bits != 8 && db_bits != 16) return VIPIR_ERR_INVALID_ARG;
+    const uint32_t n_moduli = mod ? mod->count : 0;
+    if (n_moduli > VIPIR_MAX_MODULI) return VIPIR_ERR_INVALID_ARG;
+    if (n_moduli > 0 && !mod->moduli) return VIPIR_ERR_INVALID_ARG;
+    for (uint32_t t = 0; t < n_moduli; ++t)
+        if (mod->moduli[t] < 2 || mod->moduli[t] >= (1u << 30)) return VIPIR_ERR_INVALID_ARG;
+    const uint32_t dl = db_bits / 8;
+    if (cols > (1ull << 31) || (cols * dl) % 16 != 0) return VIPIR_ERR_UNSUPPORTED;
+    const uint64_t kbytes = cols * dl;
+    if (rows >= (1ull << 31) || kbytes >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    const uint32_t T = n_moduli ? n_moduli : 1;
+    if ((uint64_t)T * batch * 5 >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    const uint32_t nq = T * batch;
+    const uint32_t lc = (dl == 2 && n_moduli > 0) ? 5u : 4u;
+    // ---- the one limit of this entry point: the limb planes have to fit the built-in array ----
+    const uint64_t planes_bytes = (uint64_t)nq * lc * kbytes;
+    if (planes_bytes > VIPIR_STATIC_SCRATCH_BYTES) {
+        snprintf(g_cuda_err, sizeof g_cuda_err,
+                 "vipir_dbmul_static: the query limb planes need %llu bytes (%u query vectors x %u limb columns x %llu "
+                 "row bytes), the built-in scratch holds VIPIR_STATIC_SCRATCH_BYTES = %u; use a plan for this size",
+                 (unsigned long long)planes_bytes, nq, lc, (unsigned long long)kbytes, (unsigned)VIPIR_STATIC_SCRATCH_BYTES);
+        return VIPIR_ERR_UNSUPPORTED;
+    }
+    // ---- per-device set-up (first call on this device only) ----
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return VIPIR_ERR_UNSUPPORTED;
+    unsigned char* scratch = nullptr;
+    int sms = 0;
+    int rc = static_scratch_setup(dev, &scratch, &sms);
+    if (rc != VIPIR_OK) return rc;
+    if ((2 + (size_t)sms) * sizeof(uint32_t) > kStaticSyncBytes) return VIPIR_ERR_UNSUPPORTED;
+
+    // A plan that lives on this stack frame and points into the static array: nothing to allocate, nothing to free
+    // (vipir_destroy must never see it).  The planner below is the one vipir_dbmul_plan uses; with d_sync already
+    // set it skips its own cudaMalloc.
+    vipir_plan pl;
+    memset(&pl, 0, sizeof pl);
+    pl.rows = rows;
+    pl.cols = cols;
+    pl.kbytes = kbytes;
+    pl.batch = batch;
+    pl.db_bits = db_bits;
+    pl.dl = dl;
+    pl.kdl = dl;
+    pl.db_layout = VIPIR_DB_ROW_MAJOR;
+    pl.n_moduli = n_moduli;
+    for (uint32_t t = 0; t < n_moduli; ++t) pl.moduli[t] = mod->moduli[t];
+    pl.nq = nq;
+    pl.lc = lc;
+    pl.num_sms = sms;
+    pl.regime = ((uint64_t)nq * lc > 64 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
+    pl.planes_bytes = planes_bytes;
+    pl.d_sync = reinterpret_cast<uint32_t*>(scratch);
+    pl.d_planes = scratch + kStaticSyncBytes;
+    rc = plan_gemm(&pl, pl.regime == VIPIR_REGIME_MMA_2SM ? 2 : 1);
+    if (rc != VIPIR_OK) return rc;
+
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // The array keeps whatever the previous call (or a call that was cut short) left in it.  The kernel expects its
+    // counters to start at zero, so they are cleared on the caller's stream ahead of the kernel.  The planes need no
+    // clearing: the splitter rewrites every byte the kernel will read.
+    CK(cudaMemsetAsync(scratch, 0, kStaticSyncBytes, st));
+    rc = launch_split(&pl, d_query, pl.d_planes, st);
+    if (rc != VIPIR_OK) return rc;
+    return scan_only(&pl, d_db, d_answer, st);
+}
 
 #include "modgemm_host.cuh"  // vipir_modgemm_* (parallel INT32 modular GEMMs, NEXT-4)
 #include "ntt_host.cuh"      // vipir_ntt_* (lift + forward NTT producing G and H)

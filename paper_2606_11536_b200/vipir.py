@@ -25,7 +25,7 @@ MAX_MODULI = 4
 # every symbol include/vipir.h declares
 SYMBOLS = (
     "vipir_dbmul_plan", "vipir_dbmul_plan_ex", "vipir_dbmul_plan_layout", "vipir_dbmul_plan_tuned", "vipir_db_split_u16",
-    "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan",
+    "vipir_dbmul", "vipir_dbmul_host", "vipir_split_limbs", "vipir_dbmul_scan", "vipir_dbmul_static",
     "vipir_plan_set_modswitch", "vipir_plan_set_db_signed",
     "vipir_plan_info", "vipir_destroy", "vipir_status_str", "vipir_last_cuda_error",
     "vipir_modgemm_plan_create", "vipir_modgemm_plan_create_tuned", "vipir_modgemm_set_h", "vipir_modgemm",
@@ -124,6 +124,8 @@ def load() -> ctypes.CDLL:
         lib.vipir_db_split_u16.argtypes = [vp, vp, u64, u64, vp]
         lib.vipir_dbmul.restype = i
         lib.vipir_dbmul.argtypes = [vp, vp, vp, vp, vp]
+        lib.vipir_dbmul_static.restype = i
+        lib.vipir_dbmul_static.argtypes = [u64, u64, u32, u32, ms, vp, vp, vp, vp]
         lib.vipir_dbmul_host.restype = i
         lib.vipir_dbmul_host.argtypes = [vp, vp, vp, vp, vp]
         lib.vipir_split_limbs.restype = i
@@ -236,6 +238,32 @@ def dbmul_host(plan, d_db, h_query, h_answer, stream=None):
     """vipir_dbmul_host: host query in, host answer out; synchronises the stream."""
     _check(load().vipir_dbmul_host(plan, _ptr(d_db), _ptr(h_query), _ptr(h_answer), _stream_ptr(stream)),
            "vipir_dbmul_host")
+
+
+STATIC_SCRATCH_BYTES = 8 << 20  # VIPIR_STATIC_SCRATCH_BYTES
+
+
+def dbmul_static(rows: int, cols: int, batch: int, d_db, d_query, d_answer, db_bits: int = 8, moduli=None, stream=None):
+    """vipir_dbmul_static: the batched product without a plan, for callers that may not allocate device memory
+    (a server whose GPU memory is fully handed out at start-up, a request path that cannot afford the device-wide
+    stall of cudaMalloc / cudaFree).  The kernel's scratch is a fixed 8 MiB array inside the library, shared by every
+    call on the GPU: the query limb planes (T * batch * LC * cols * db_bits/8 bytes) must fit in
+    STATIC_SCRATCH_BYTES, else VipirError(ERR_UNSUPPORTED) with the two sizes in the message; calls whose GPU work
+    overlaps race.  The first call on a device does a one-time address look-up: make it before any stream capture.
+    Only enqueues on `stream` (default: torch's current stream); same answer as dbmul, bit for bit."""
+    lib = load()
+    spec_p = None
+    if moduli is not None and len(moduli) > 0:
+        arr = (ctypes.c_uint32 * len(moduli))(*[int(m) for m in moduli])
+        spec = ModulusSpec(len(moduli), arr)
+        spec_p = ctypes.byref(spec)
+    status = lib.vipir_dbmul_static(rows, cols, batch, db_bits, spec_p, _ptr(d_db), _ptr(d_query), _ptr(d_answer),
+                                    _stream_ptr(stream))
+    if status == ERR_UNSUPPORTED:
+        why = lib.vipir_last_cuda_error().decode()
+        if why:
+            raise VipirError(status, why)
+    _check(status, "vipir_dbmul_static")
 
 
 def split_limbs(plan, d_query, d_planes_out=None, stream=None):
