@@ -2,9 +2,10 @@
 
 All work is integer, so the bar is exact equality of every compared word (no tolerance).
 Small and medium shapes are compared in full and are sized to span several tiles plus a
-ragged tail in every dimension (rows, K bytes, query vectors, K chunks); BASELINE.json's
-full-size configs are compared on sampled rows the oracle computes one by one, plus a
-column-sum identity that covers every row at any size (tests/test_parity_fullsize_gpu.py).
+ragged tail in every dimension (rows, K bytes, query vectors, K chunks).  BASELINE.json's
+full-size configs are in tests/test_parity_fullsize_gpu.py: configs[1] and configs[2] at B = 1 in full,
+the batched ones on whole 128-row tiles plus a column-sum identity over every row, through both the
+device and the host entry point.
 """
 import os
 
@@ -474,6 +475,47 @@ def test_host_entry_point_tensor_regimes(name, rows, cols, batch, bits, moduli, 
         pinned.fill_(-1)
         plan.host(d_db, h_q, pinned[:T * batch * rows])
         assert_same(pinned[:T * batch * rows].numpy().view(np.uint32).reshape(T, batch, rows), want)
+
+
+def test_host_entry_point_at_scale_planner_slices_several_units_per_cta():
+    """The server's per-request path (PAPER.md:117 "a D1 x B x D0 ... GEMM for a batch of B queries", :176 the DB
+    resident in GPU DRAM) at a size where nothing is forced: 60000 x 8192 u8, B = 256, regime AUTO.  The query is
+    8 MiB, so the planner's own rule cuts the call into three K slices; there are several times more work units
+    than CTA pairs, so every pair finishes several units per slice -- its two-entry copier ring wraps and its copier
+    warps run behind its epilogue warps -- and the rows end in a ragged tile.  The answer, delivered into mapped
+    host memory, is compared with the oracle on the first, the last (ragged) and 16 seeded random 128-row tiles,
+    all 256 query vectors; the same call into pageable memory and the device call must give the same words
+    everywhere."""
+    import torch
+    from paper_2606_11536_b200.inputs import device
+    ensure_built()
+    rows, cols, batch, seed = 60000, 8192, 256, 123
+    d_db = device.db(seed, rows, cols, 8)
+    Q = inputs.query(seed, cols, batch, None)
+    assert Q.nbytes == 8 << 20  # the planner's three-slice threshold (no host_slices forced)
+    h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+    h_a = torch.full((1, batch, rows), -1, dtype=torch.int32).pin_memory()
+    pageable = torch.full((1, batch, rows), -1, dtype=torch.int32)
+    d_a = torch.full((1, batch, rows), -1, dtype=torch.int32, device="cuda")
+    with vipir.Plan(rows, cols, batch) as plan:
+        i = plan.info
+        assert i["regime_name"] == "mma_2sm"
+        assert i["n_tiles"] * i["m_tiles"] >= 6 * i["grid"] // 2, i  # >= 6 finished units per CTA pair
+        plan.host(d_db, h_q, h_a)
+        plan.host(d_db, h_q, pageable)
+        plan(d_db, torch.from_numpy(Q.view(np.int32)).cuda(), d_a)
+        torch.cuda.synchronize()
+    got = h_a.numpy().view(np.uint32)
+    n_tiles = (rows + 127) // 128
+    tiles = sorted({0, n_tiles - 1, *np.random.default_rng(seed).choice(n_tiles, size=16, replace=False).tolist()})
+    assert np.array_equal(d_db[777].cpu().numpy(), inputs.db_rows(seed, rows, cols, 8, row0=777, nrows=1)[0])
+    for t0 in tiles:
+        r0, r1 = t0 * 128, min(rows, t0 * 128 + 128)
+        want = oracle.dbmul(d_db[r0:r1].cpu().numpy(), Q, None, nthreads=NT)
+        assert_same(got[:, :, r0:r1], want)
+    assert (got[:, :, rows - 96:] != 0xFFFFFFFF).any()  # the ragged tile was written
+    assert np.array_equal(pageable.numpy().view(np.uint32), got), "pageable and mapped host answers differ"
+    assert np.array_equal(d_a.cpu().numpy().view(np.uint32), got), "host and device entry points differ"
 
 
 def test_forced_chunk_count_that_does_not_divide_the_k_atoms():
