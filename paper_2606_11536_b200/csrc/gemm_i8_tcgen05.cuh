@@ -450,7 +450,10 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 const uint32_t want = c * GM_EPI_WARPS * CG;
                 const long long t0 = clock64();
                 while (ptx::ld_acquire_gpu(cnt) < want) {
-                    if (clock64() - t0 > (20ll << 30)) __trap();  // ~10 s: never in a correct run
+                    // a bound far above any legitimate wait: the longest one is a single unit cut into 65536 chunks
+                    // (rows <= 128, K = 2^31 - 16: tests/test_max_sizes_gpu.py), whose chunks are accumulated strictly
+                    // in order, group after group -- 7-11 s on a B200, which the former ~11 s bound cut short on some runs
+                    if (clock64() - t0 > (1ll << 38)) __trap();  // ~2.4 min at 1.9 GHz: never in a correct run
                 }
             }
             // later chunks add to what chunk 0 stored: a fire-and-forget red.add for q = 2^32; for
