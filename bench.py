@@ -243,10 +243,15 @@ def two_in_flight(rows, cols, batch, db_bits, moduli, layout, d_db, h_q, d_ref, 
     return max(ms) / (2 * steps)
 
 
-def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset_bytes=0, spread=False):
+MIN_WINDOW_MS = 100.0  # a step under 2 ms is timed over at least this long a window (the clock oscillates at the power cap)
+
+
+def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset_bytes=0, spread=False, exact_steps=False):
     """Times one config on the current device; returns a dict of measurements.  Every config that runs on the tensor
     cores is timed in the power-capped steady state (a 1 s settle loop first: `ms_per_step`, the number of record)
-    and as a burst (`ms_per_step_burst`: the first steps after 0.5 s of idle)."""
+    and as a burst (`ms_per_step_burst`: the first steps after 0.5 s of idle).  Unless exact_steps (the headline: the
+    contract's exactly-K steps), whatever takes under 2 ms per call is re-timed over a window of >= MIN_WINDOW_MS
+    (`timed_steps` says how many calls that was), the step, the scan kernel and the splitter alike."""
     import torch
     from paper_2606_11536_b200 import inputs, vipir
     from paper_2606_11536_b200.inputs import device
@@ -283,15 +288,22 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
             time.sleep(0.5)
             out["ms_per_step_burst"] = time_events(lambda: plan(d_db, d_q, d_a), 3, 0, stream) / 3
             settle(lambda: plan(d_db, d_q, d_a))
-        ms_step = time_events(lambda: plan(d_db, d_q, d_a), steps, warmup, stream) / steps
+        def timed(fn):
+            ms = time_events(fn, steps, warmup, stream) / steps
+            n = steps
+            if not exact_steps and ms < 2.0 and ms * steps < MIN_WINDOW_MS:
+                n = int(MIN_WINDOW_MS / max(ms, 1e-3)) + 1
+                ms = time_events(fn, n, 0, stream) / n
+            return ms, n
+        ms_step, out["timed_steps"] = timed(lambda: plan(d_db, d_q, d_a))
         if spread:  # headline config: spread of the single steps as well
             out["ms_step_spread"] = step_spread(lambda: plan(d_db, d_q, d_a), min(steps, 50), stream)
         # the dominant kernel alone (planes already in the workspace) and the splitter alone
         if info["launches"] == 1:   # GEMV with the split fused in: the step IS the scan kernel (same timed region)
             ms_scan = ms_step
         else:
-            ms_scan = time_events(lambda: vipir.dbmul_scan(plan.handle, d_db, d_a), steps, warmup, stream) / steps
-        ms_split = time_events(lambda: vipir.split_limbs(plan.handle, d_q), steps, warmup, stream) / steps
+            ms_scan, _ = timed(lambda: vipir.dbmul_scan(plan.handle, d_db, d_a))
+        ms_split, _ = timed(lambda: vipir.split_limbs(plan.handle, d_q))
         if with_e2e:
             # the public host call (vipir_dbmul_host): query from pinned host memory in, answer in host memory out,
             # stream sync -- every step; the tensor regimes pipeline it over K slices (include/vipir.h)
@@ -324,6 +336,9 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
     nq, lc = info["query_vectors"], info["limb_cols"]
     logical_ops = 2.0 * rows * cols * nq
     int8_ops = 2.0 * rows * kb * nq * lc  # what the tensor pipe executes (limb MACs)
+    # what the method asks for: four query limbs x the DB element's byte limbs per product -- 4 int8
+    # MACs for a u8 DB, 8 for u16; the byte view of a u16 DB executes 10
+    method_ops = 2.0 * rows * cols * nq * 4 * (db_bits // 8)
     alg_bytes = db_bytes + 4 * cols * nq + 4 * rows * nq  # DB + query + answer
     out.update({
         "regime": info["regime_name"], "ms_per_step": ms_step, "ms_scan_kernel": ms_scan, "ms_split_kernel": ms_split,
@@ -333,11 +348,16 @@ def run_config(name, device_db, steps, warmup, peaks, with_e2e=False, row_offset
         "frac_hbm_measured": alg_bytes / ms_scan / 1e6 / peaks["hbm_gbs"],
         "frac_hbm_nominal_8TBps": db_bytes / ms_step / 1e6 / 8000.0,
         "frac_int8_nominal_4500": int8_ops / ms_step / 1e9 / 4500.0,
-        "frac_int8_measured_sustained": int8_ops / ms_scan / 1e9 / (2.0 * peaks["bf16_sustained"]),
         "plan": {k: info[k] for k in ("tile_cols", "mma_n", "m_tiles", "n_tiles", "n_chunks", "k_chunk_bytes", "stages",
                                        "grid", "smem_bytes", "launches")},
-        "alg_bytes": alg_bytes, "int8_ops": int8_ops,
+        "alg_bytes": alg_bytes, "int8_ops": int8_ops, "method_int8_ops": method_ops,
     })
+    if tensor and peaks.get("mma_i8_sustained_TOPS"):
+        # the scan kernel against the int8 MMA ceiling measured live in this run (ceilings.cu, sustained): the limb MACs
+        # it executes, and the method's own (what the answer needs)
+        ceil = peaks["mma_i8_sustained_TOPS"]
+        out["frac_mma_ceiling_executed"] = int8_ops / ms_scan / 1e9 / ceil
+        out["frac_mma_ceiling_method"] = method_ops / ms_scan / 1e9 / ceil
     del d_q, d_a
     return out
 
@@ -611,7 +631,7 @@ def run_cuda(args):
     # ---- headline: timed region bracketed by barrier + synchronize, clocks sampled during it ----
     barrier()
     with ClockSampler(local_rank) as clk:
-        head = run_config(HEADLINE, buf, args.steps, args.warmup, peaks, with_e2e=True, spread=True)
+        head = run_config(HEADLINE, buf, args.steps, args.warmup, peaks, with_e2e=True, spread=True, exact_steps=True)
     barrier()
     times = [head["ms_per_step"] * args.steps]
     e2e_times = [head["e2e_ms"] * args.steps]
@@ -632,12 +652,26 @@ def run_cuda(args):
     mma_ceil = None
     if rank == 0 and world == 1:
         mma_ceil = mma_i8_ceiling()
+        peaks["mma_i8_sustained_TOPS"] = mma_ceil["sustained_TOPS"]
         # every BASELINE.json config rides along at N = 1 (a few seconds); --headline-only keeps just configs[2] and [3]
         for name in ([BATCHED] if args.headline_only else [n for n in CONFIGS if n != HEADLINE]):
             extra[name] = run_config(name, buf, args.steps, max(3, args.warmup), peaks, with_e2e=(name == BATCHED))
         if args.paper:
+            # the read-only ceiling on the buffer each paper workload scans (the 64 GiB ones against 64 GiB of loads:
+            # TLB reach and refresh are the part's, whatever they cost)
+            ro = {}
+            for label, nb in (("16GiB", 16 << 30), ("64GiB", 64 << 30)):
+                if nb <= alloc_bytes:
+                    ms = time_events(lambda: device.read_only(buf[:nb]), 5, 2, torch.cuda.current_stream()) / 5
+                    ro[label] = nb / ms / 1e6
+            extra["paper_read_only"] = {"GBps": ro, "how": "plain 128-bit loads over the first 16 / 64 GiB of the same buffer, 5 passes"}
             for name in PAPER_CONFIGS:
                 extra[name] = run_config(name, buf, max(10, args.steps // 5), 3, peaks)
+                r_, c_, _, bits_, _ = PAPER_CONFIGS[name]
+                label = {16 << 30: "16GiB", 64 << 30: "64GiB"}.get(r_ * c_ * bits_ // 8)
+                if label in ro:
+                    extra[name]["read_only_ceiling_GBps"] = ro[label]
+                    extra[name]["frac_of_read_only_ceiling"] = extra[name]["scan_kernel_GBps"] / ro[label]
                 if name in PAPER_QPS_H100:
                     extra[name]["qps_batch32"] = 32.0 / (extra[name]["ms_per_step"] * 1e-3)
                     extra[name]["paper_qps_h100_nvl"] = PAPER_QPS_H100[name]
@@ -646,7 +680,7 @@ def run_cuda(args):
         if not args.headline_only or args.modgemm:
             mg_B = (1, 8, 32) if args.modgemm else (32,)
             extra["modgemm"] = {f"B{B}": run_modgemm(B, max(10, args.steps // 5), 3, peaks) for B in mg_B}
-            extra["ntt"] = {"G_B32": run_ntt(32, "G", 50, 5)}
+            extra["ntt"] = {"G_B32": run_ntt(32, "G", 300, 5)}  # ~0.4 ms per launch: a window above 100 ms
             if args.modgemm:
                 extra["ntt"].update({"G_B1": run_ntt(1, "G", 50, 5), "H_n1280_offline": run_ntt(1280, "H", 3, 1)})
         if args.pipeline:
@@ -657,6 +691,80 @@ def run_cuda(args):
 
     if rank == 0:
         b = extra.get(BATCHED)
+        roofline = {"bound": "hbm", "kernel": "gemv_b1_kernel", "achieved": head["scan_kernel_GBps"],
+                    "peak": peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)"
+                    if peaks["source"] == "measured" else "fallback 6650 GB/s (B200_PROFILING.md)",
+                    "unit": "GB/s", "frac": head["frac_hbm_measured"],
+                    "frac_of_nominal_8TBps": head["scan_kernel_GBps"] / 8000.0,
+                    "read_only_ceiling_GBps": read_only_gbs,
+                    "frac_of_read_only_ceiling": head["scan_kernel_GBps"] / read_only_gbs,
+                    "ms_per_launch": head["ms_scan_kernel"], "alg_bytes_per_launch": head["alg_bytes"],
+                    "traffic": profiled_traffic("gemv_b1_kernel")}
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": head["h2d_bytes"],
+               "d2h_bytes_per_step": head["d2h_bytes"], "ms_per_step": head["e2e_ms"]}
+        batched = None
+        if b:
+            sus = mma_ceil["sustained_TOPS"]
+            batched = {
+                "workload": "configs[3]: 4 GiB u8 DB 65536x65536, Q 65536x256 u32, q=2^32, 4 int8 limbs, K chunks <= 32768",
+                "ms_per_step": b["ms_per_step"], "ms_per_step_burst": b["ms_per_step_burst"],
+                "db_GBps": b["db_GBps"], "logical_TOPS": b["logical_TOPS"],
+                "int8_TOPS": b["int8_TOPS"], "regime": b["regime"],
+                "e2e": {"ms_per_step": b["e2e_ms"], "int8_TOPS": b["int8_ops"] / b["e2e_ms"] / 1e9,
+                        "db_GBps": b["rows"] * b["cols"] / b["e2e_ms"] / 1e6,
+                        "ratio_to_device_step": b["e2e_ms"] / b["ms_per_step"],
+                        "two_requests_in_flight": {
+                            "ms_per_request": b["e2e_two_in_flight_ms"],
+                            "ratio_to_device_step": b["e2e_two_in_flight_ms"] / b["ms_per_step"],
+                            "how": "two host threads, each with its own plan, stream and pinned buffers, calling "
+                                   "vipir_dbmul_host back to back on the same resident DB"},
+                        "h2d_bytes_per_step": b["h2d_bytes"], "d2h_bytes_per_step": b["d2h_bytes"],
+                        "pcie_h2d_GBps": b["pcie_h2d_GBps"], "pcie_d2h_GBps": b["pcie_d2h_GBps"],
+                        "how": "vipir_dbmul_host: H2D, limb split and scan pipelined over K slices, the answer "
+                               "copied into mapped pinned host memory tile by tile; sustained (1 s settle)"},
+                "roofline": {"bound": "tensor", "kernel": "gemm_i8_kernel<2,4,false>", "achieved": b["scan_kernel_int8_TOPS"],
+                             "peak": sus, "unit": "TOP/s (int8)",
+                             "peak_source": "measured live, sustained: pure tcgen05.mma.kind::i8 loop (ceilings.cu); "
+                                            + mma_ceil["how"],
+                             "frac": b["scan_kernel_int8_TOPS"] / sus,
+                             "int8_mma_ceiling_TOPS": {"burst": mma_ceil["burst_TOPS"], "sustained": sus},
+                             "achieved_burst": b["int8_ops"] / b["ms_per_step_burst"] / 1e9,
+                             "frac_burst_of_burst_ceiling": b["int8_ops"] / b["ms_per_step_burst"] / 1e9 / mma_ceil["burst_TOPS"],
+                             "frac_of_nominal_4500": b["scan_kernel_int8_TOPS"] / 4500.0,
+                             "frac_of_2x_measured_sustained_bf16": b["scan_kernel_int8_TOPS"] / (2.0 * peaks["bf16_sustained"]),
+                             "ms_per_launch": b["ms_scan_kernel"], "int8_ops_per_launch": b["int8_ops"],
+                             "traffic": profiled_traffic("gemm_i8_kernel")},
+            }
+            # compact copies inside the two objects every record of this line keeps whole (`roofline`, `e2e`)
+            br = batched["roofline"]
+            roofline["batched"] = {
+                "workload": "configs[3] 4 GiB u8, B = 256", "bound": "tensor", "kernel": br["kernel"],
+                "achieved": br["achieved"], "peak": br["peak"], "unit": br["unit"],
+                "peak_source": "int8 MMA ceiling measured live, sustained (ceilings.cu)", "frac": br["frac"],
+                "frac_of_nominal_4500": br["frac_of_nominal_4500"], "ms_per_launch": br["ms_per_launch"],
+                "ms_per_step": b["ms_per_step"], "ms_per_step_burst": b["ms_per_step_burst"], "traffic": br["traffic"]}
+            e2e["batched"] = {
+                "ms_per_step": b["e2e_ms"], "ratio_to_device_step": b["e2e_ms"] / b["ms_per_step"],
+                "two_in_flight_ms": b["e2e_two_in_flight_ms"], "h2d_bytes_per_step": b["h2d_bytes"],
+                "d2h_bytes_per_step": b["d2h_bytes"]}
+            for key, cname in (("configs4_byte_view", "C5_rns_u16_B64x2"), ("configs4_limb_planes", "C5_rns_u16_B64x2_planes")):
+                c = extra.get(cname)
+                if c:
+                    roofline[key] = {"bound": "tensor", "ms_per_step": c["ms_per_step"], "ms_per_launch": c["ms_scan_kernel"],
+                                     "peak": sus, "unit": "TOP/s (int8)", "achieved_executed": c["scan_kernel_int8_TOPS"],
+                                     "achieved_method": c["method_int8_ops"] / c["ms_scan_kernel"] / 1e9,
+                                     "frac_executed": c["frac_mma_ceiling_executed"], "frac": c["frac_mma_ceiling_method"]}
+        mg32 = extra.get("modgemm", {}).get("B32")
+        if mg32:
+            r = mg32["roofline"]
+            roofline["modgemm_B32"] = {k: r[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "ms_per_launch",
+                                                          "traffic")}
+        ntt32 = extra.get("ntt", {}).get("G_B32")
+        if ntt32:
+            r = ntt32["roofline"]
+            roofline["ntt_G_B32"] = {"bound": r["bound"], "kernel": r["kernel"], "achieved": r["achieved"], "peak": r["peak"],
+                                     "unit": r["unit"], "frac": r["frac"], "ms_per_launch": ntt32["ms"], "traffic": r["traffic"]}
+        # key order: the per-config detail first, the objects of record last (a truncated tail of the line still holds them)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -665,65 +773,23 @@ def run_cuda(args):
                                    "seed 0; per GPU (row-sharded for N>1)",
                        "regime": head["regime"], "l2": "inputs (16 GiB) larger than L2; no flush",
                        "plan": head["plan"]},
-            "clocks": clk.summary(),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": head["h2d_bytes"],
-                    "d2h_bytes_per_step": head["d2h_bytes"], "ms_per_step": head["e2e_ms"]},
-            "gpu_launches": head["plan"]["launches"] * args.steps,
-            "ms_per_step_spread": head.get("ms_step_spread"),
-            "roofline": {"bound": "hbm", "kernel": "gemv_b1_kernel", "achieved": head["scan_kernel_GBps"],
-                         "peak": peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)"
-                         if peaks["source"] == "measured" else "fallback 6650 GB/s (B200_PROFILING.md)",
-                         "unit": "GB/s", "frac": head["frac_hbm_measured"],
-                         "frac_of_nominal_8TBps": head["scan_kernel_GBps"] / 8000.0,
-                         "read_only_ceiling_GBps": read_only_gbs,
-                         "frac_of_read_only_ceiling": head["scan_kernel_GBps"] / read_only_gbs,
-                         "ms_per_launch": head["ms_scan_kernel"], "alg_bytes_per_launch": head["alg_bytes"],
-                         "traffic": profiled_traffic("gemv_b1_kernel")},
-            "cpu_baseline": cpu,
         }
-        if b:
-            sus = mma_ceil["sustained_TOPS"]
-            line["batched"] = {
-                "workload": "configs[3]: 4 GiB u8 DB 65536x65536, Q 65536x256 u32, q=2^32, 4 int8 limbs, K chunks <= 32768",
-                "ms_per_step": b["ms_per_step"], "ms_per_step_burst": b["ms_per_step_burst"],
-                "db_GBps": b["db_GBps"], "logical_TOPS": b["logical_TOPS"],
-                "int8_TOPS": b["int8_TOPS"], "regime": b["regime"], "plan": b["plan"],
-                "e2e": {"ms_per_step": b["e2e_ms"], "int8_TOPS": b["int8_ops"] / b["e2e_ms"] / 1e9,
-                        "db_GBps": b["rows"] * b["cols"] / b["e2e_ms"] / 1e6,
-                        "ratio_to_device_step": b["e2e_ms"] / b["ms_per_step"],
-                        "two_requests_in_flight": {
-                            "ms_per_request": b["e2e_two_in_flight_ms"],
-                            "ratio_to_device_step": b["e2e_two_in_flight_ms"] / b["ms_per_step"],
-                            "how": "two host threads, each with its own plan, stream and pinned buffers, calling "
-                                   "vipir_dbmul_host back to back on the same resident DB: one request's copies run "
-                                   "beside the other's scan (throughput of a server that overlaps requests)"},
-                        "h2d_bytes_per_step": b["h2d_bytes"], "d2h_bytes_per_step": b["d2h_bytes"],
-                        "pcie_h2d_GBps": b["pcie_h2d_GBps"], "pcie_d2h_GBps": b["pcie_d2h_GBps"],
-                        "how": "vipir_dbmul_host: H2D, limb split and scan pipelined over K slices, the answer "
-                               "stored into mapped pinned host memory by the last slice; sustained (1 s settle)"},
-                "roofline": {"bound": "tensor", "kernel": "gemm_i8_kernel<2,4,false>", "achieved": b["scan_kernel_int8_TOPS"],
-                             "peak": sus, "unit": "TOP/s (int8)",
-                             "peak_source": "measured live, sustained: pure tcgen05.mma.kind::i8 loop (ceilings.cu); "
-                                            + mma_ceil["how"],
-                             "frac": b["scan_kernel_int8_TOPS"] / sus,
-                             "int8_mma_ceiling_TOPS": {"burst": mma_ceil["burst_TOPS"], "sustained": sus},
-                             "frac_of_int8_mma_ceiling": b["scan_kernel_int8_TOPS"] / sus,
-                             "achieved_burst": b["int8_ops"] / b["ms_per_step_burst"] / 1e9,
-                             "frac_burst_of_burst_ceiling": b["int8_ops"] / b["ms_per_step_burst"] / 1e9 / mma_ceil["burst_TOPS"],
-                             "frac_of_nominal_4500": b["scan_kernel_int8_TOPS"] / 4500.0,
-                             "frac_of_2x_measured_sustained_bf16": b["frac_int8_measured_sustained"],
-                             "ms_per_launch": b["ms_scan_kernel"], "int8_ops_per_launch": b["int8_ops"],
-                             "traffic": profiled_traffic("gemm_i8_kernel")},
-            }
-        if "modgemm" in extra:
-            line["modgemm"] = extra.pop("modgemm")
-        if "ntt" in extra:
-            line["ntt"] = extra.pop("ntt")
-        if "pipeline" in extra:
-            line["pipeline"] = extra.pop("pipeline")
+        if extra.get("paper_read_only"):
+            line["paper_read_only_ceiling"] = extra.pop("paper_read_only")
+        for key in ("modgemm", "ntt", "pipeline"):
+            if key in extra:
+                line[key] = extra.pop(key)
         if extra:
-            line["configs"] = {n: {k: v for k, v in r.items() if k != "alg_bytes"} for n, r in extra.items()}
-            line["configs"][HEADLINE] = {k: v for k, v in head.items() if k != "alg_bytes"}
+            drop = ("alg_bytes", "plan")
+            line["configs"] = {n: {k: v for k, v in r.items() if k not in drop} for n, r in extra.items()}
+            line["configs"][HEADLINE] = {k: v for k, v in head.items() if k not in drop}
+        if batched:
+            line["batched"] = batched
+        line.update({
+            "clocks": clk.summary(), "gpu_launches": head["plan"]["launches"] * args.steps,
+            "ms_per_step_spread": head.get("ms_step_spread"),
+            "cpu_baseline": cpu, "e2e": e2e, "roofline": roofline,
+        })
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -769,7 +835,6 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--all", action="store_true", help="(default since r01j) time every BASELINE.json config at N = 1")
     ap.add_argument("--headline-only", action="store_true", help="time only configs[2] (headline) and configs[3] (batched)")
     ap.add_argument("--paper", action="store_true", help="also time the paper's Table-2 shapes and NEXT-2 shapes (64 GiB DB)")
     ap.add_argument("--modgemm", action="store_true",
