@@ -165,7 +165,7 @@ typedef struct {
     uint32_t host_staged;    /* vipir_dbmul_host: 1 = always stage the answer in device memory and copy it back
                                 (no direct stores into mapped host memory, no overlapped copies) */
     uint32_t host_slices;    /* vipir_dbmul_host, MMA: K slices of the copy / split / scan pipeline, 1..4 (0: three for
-                                queries of 8 MiB and more, else one) */
+                                queries of 8 MiB and more, else one); UNSUPPORTED for a GEMV plan */
     uint32_t reserved[6];    /* must be 0 */
 } vipir_tuning;
 
@@ -329,8 +329,12 @@ const char *vipir_last_cuda_error(void);
  * Ownership: the caller owns all four; the plan owns a re-laid-out byte-limb copy of H
  * (4*T*NC*M*Kp bytes, Kp = K rounded up to 128; written by vipir_modgemm_set_h, after which the
  * caller may free d_H) and the limb planes of C (4*T*NC*ncols*Kp bytes, rewritten every call).
- * Execution and errors as for vipir_dbmul: calls only enqueue on `cuda_stream`; one plan must
- * not be in flight on two streams.
+ * Execution and errors as for vipir_dbmul: calls only enqueue on `cuda_stream`.  One plan must not be in flight
+ * on two streams, nor be used from two host threads at once: vipir_modgemm keeps per-plan state between calls --
+ * the tensor map of the caller's C is cached for the last d_C seen and re-encoded (a host-side call of a few
+ * microseconds) whenever d_C changes, so a caller that alternates C buffers may prefer one plan per buffer; and the
+ * C limb planes of the two-kernel form are allocated by the plan call when that is the plan's form, else by the
+ * first vipir_modgemm_split_c (ALLOC can come from there).  A server that overlaps requests makes one plan per stream.
  * =========================================================================================== */
 typedef struct vipir_modgemm_plan vipir_modgemm_plan;
 
@@ -359,7 +363,9 @@ typedef struct {
     uint32_t b_stages;    /* ring depth of the C operand: 2..4 */
     uint32_t c_split;     /* where vipir_modgemm splits C into limbs: 1 = a splitter kernel of its own (two launches),
                              2 = inside the products kernel (one launch; UNSUPPORTED unless K % 4 == 0) */
-    uint32_t r_stages;    /* fused form: ring depth of the raw C tiles, 2..4 */
+    uint32_t r_stages;    /* one-kernel form: ring depth of the raw C tiles, 2..4; UNSUPPORTED when the plan's form is two
+                             kernels.  (a_stages and b_stages apply to whichever form runs, and to both when the parts
+                             are called on a one-kernel plan.) */
     uint32_t reserved[2]; /* must be 0 */
 } vipir_modgemm_tuning;
 

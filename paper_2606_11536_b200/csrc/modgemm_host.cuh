@@ -15,7 +15,7 @@ struct vipir_modgemm_plan {
     uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
     uint64_t hp_bytes, cp_bytes;
     bool h_set;
-    bool fused;          // vipir_modgemm splits C inside the products kernel (from 32 columns up, K % 4 == 0): one launch
+    bool fused;          // vipir_modgemm splits C inside the products kernel (from 16 columns up and K % 4 == 0): one launch
     vipir::ModGemmParams mg, mg_fused;
     uint32_t smem_bytes, smem_bytes_fused, grid;
     CUtensorMap tm_h, tm_c;
@@ -109,6 +109,9 @@ int plan_modgemm(vipir_modgemm_plan* p) {
         g.barrett[t] = (uint64_t)((((unsigned __int128)1) << 64) / q);
     }
     p->smem_bytes = g.a_stages * vipir::MG_A_BYTES + g.b_stages * g.b_stage_bytes + overhead;
+    // (The two-kernel parameters above are planned and checked for every plan -- vipir_modgemm_split_c + _products may be
+    // called on a one-kernel plan too.  That never refuses a shape or an override the one-kernel form could run: the
+    // two-kernel form has no raw ring and at most as many operand slots, so whenever the checks below pass, those did.)
     // the fused kernel: two operand slots, two to four raw-tile slots (ct columns x 128 words each), the rest to the H ring
     p->mg_fused = g;
     if (p->fused) {
@@ -268,6 +271,10 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
         return VIPIR_ERR_UNSUPPORTED;
     }
     p->fused = p->tune.c_split ? p->tune.c_split == 2 : (K % 4 == 0 && ncols >= 16);
+    if (p->tune.r_stages && !p->fused) {  // the raw-tile ring exists in the one-kernel form only: refused, not ignored
+        delete p;
+        return VIPIR_ERR_UNSUPPORTED;
+    }
     p->hp_bytes = p->P * M * 4ull * p->Kp;
     p->cp_bytes = p->P * 4ull * ncols * p->Kp;
     // the C limb planes are only needed by the two-kernel form: allocated here when that is the plan's form,

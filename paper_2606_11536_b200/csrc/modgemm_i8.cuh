@@ -33,7 +33,7 @@
 //            low four sums, 2^(8s) mod q weights for the high three), + G, one Barrett reduction,
 //            store (coalesced over rows).
 //
-// FUSED (the default whenever K % 4 == 0): the limb split of C -- the paper fuses its prmt decomposition into
+// FUSED (the default from 16 columns up and K % 4 == 0): the limb split of C -- the paper fuses its prmt decomposition into
 // the GEMM kernel too -- happens inside this kernel instead of a pre-pass that writes and re-reads
 // 4 bytes per word of C.  The producer brings the RAW u32 words of the C tile by TMA (four 32-word x ct-column
 // boxes per k-atom, 128B-swizzled so that a thread's 64-byte run reads conflict-free), two converter warps

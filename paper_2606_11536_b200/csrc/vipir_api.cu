@@ -306,7 +306,7 @@ int plan_gemm(vipir_plan* p, int cg) {
 int plan_gemv(vipir_plan* p) {
     if (p->nq != 1 || p->n_moduli != 0 || p->lc != 4) return VIPIR_ERR_UNSUPPORTED;
     const vipir_tuning& tu = p->tune;  // overrides of the tensor-core regimes do not apply here
-    if (tu.m_sub || tu.tile_queries || tu.k_atoms || tu.min_chunks || tu.whole_units || tu.no_collector)
+    if (tu.m_sub || tu.tile_queries || tu.k_atoms || tu.min_chunks || tu.whole_units || tu.no_collector || tu.host_slices)
         return VIPIR_ERR_UNSUPPORTED;
     vipir::GemvParams& g = p->gv;
     memset(&g, 0, sizeof g);
@@ -629,9 +629,9 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     }
     uint32_t bounds[kMaxHostSlices + 1];
     const uint32_t S = (mma && !p->tune.host_staged) ? host_slices(p, qbytes, bounds) : 1u;
-    // the running sums between K chunks / slices are read back by the kernels: they stay in device memory
-    const bool need_stage = true;  // the kernels accumulate in device memory; the mapped host buffer only receives finished units
-    if (need_stage && !p->d_a_stage && cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
+    // the running sums between K chunks / slices are read back by the kernels: they stay in device memory (the
+    // mapped host buffer only receives finished units)
+    if (!p->d_a_stage && cudaMalloc(&p->d_a_stage, abytes) != cudaSuccess) {
         cudaGetLastError();
         return VIPIR_ERR_ALLOC;
     }
@@ -667,22 +667,37 @@ int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, u
     CK(cudaStreamWaitEvent(p->copy_stream, p->ev_begin, 0));
     uint32_t* const d_final = d_direct ? d_direct : p->d_a_stage;
     const size_t pitch = (size_t)p->cols * 4;
+    // From here on work is in flight on both streams.  The call promises to be complete when it returns, also
+    // when it fails: an error exit first waits for whatever was enqueued (copies still reading h_query, kernels
+    // still writing the staging buffers or h_answer), so the caller may free or reuse its buffers and the plan.
+    auto fail = [&](int rc) {
+        cudaStreamSynchronize(p->copy_stream);
+        cudaStreamSynchronize(st);
+        cudaGetLastError();  // the error of record is the one already in g_cuda_err
+        return rc;
+    };
+#define CKD(call)                                                   \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return fail(cuda_fail(e__, #call)); \
+    } while (0)
     for (uint32_t i = 0; i < S; ++i) {
         const uint64_t c_lo = (uint64_t)bounds[i] * vipir::GM_BK / p->kdl;
         uint64_t c_hi = (uint64_t)bounds[i + 1] * vipir::GM_BK / p->kdl;
         if (c_hi > p->cols) c_hi = p->cols;
-        CK(cudaMemcpy2DAsync(p->d_q_stage + c_lo, pitch, h_query + c_lo, pitch, (size_t)(c_hi - c_lo) * 4, p->nq,
-                             cudaMemcpyHostToDevice, p->copy_stream));
+        CKD(cudaMemcpy2DAsync(p->d_q_stage + c_lo, pitch, h_query + c_lo, pitch, (size_t)(c_hi - c_lo) * 4, p->nq,
+                              cudaMemcpyHostToDevice, p->copy_stream));
         int rc = launch_split(p, p->d_q_stage, p->d_planes, p->copy_stream, c_lo, c_hi);
-        if (rc != VIPIR_OK) return rc;
-        CK(cudaEventRecord(p->ev_slice[i], p->copy_stream));
-        CK(cudaStreamWaitEvent(st, p->ev_slice[i], 0));
+        if (rc != VIPIR_OK) return fail(rc);
+        CKD(cudaEventRecord(p->ev_slice[i], p->copy_stream));
+        CKD(cudaStreamWaitEvent(st, p->ev_slice[i], 0));
         KSlice sl{bounds[i], bounds[i + 1] - bounds[i], i > 0 ? 1u : 0u, i + 1 == S ? d_final : p->d_a_stage, i + 1 == S};
-        rc = scan_only(p, d_db, p->d_a_stage ? p->d_a_stage : d_final, st, nullptr, &sl);
-        if (rc != VIPIR_OK) return rc;
+        rc = scan_only(p, d_db, p->d_a_stage, st, nullptr, &sl);
+        if (rc != VIPIR_OK) return fail(rc);
     }
-    if (!d_direct) CK(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
+    if (!d_direct) CKD(cudaMemcpyAsync(h_answer, p->d_a_stage, abytes, cudaMemcpyDeviceToHost, st));
+    CKD(cudaStreamSynchronize(st));
+#undef CKD
     return VIPIR_OK;
 }
 

@@ -355,6 +355,17 @@ def test_tuning_overrides_are_honoured_or_refused():
     assert status(M1, separate_split=1) == vipir.ERR_UNSUPPORTED       # a GEMV override
     assert status(G, batch=1, m_sub=2) == vipir.ERR_UNSUPPORTED        # an MMA override
     assert status(G, batch=1, stages=7) == vipir.ERR_UNSUPPORTED
+    assert status(G, batch=1, host_slices=2) == vipir.ERR_UNSUPPORTED  # K slices are the tensor regimes' host pipeline
+    assert status(M1, host_slices=2) == vipir.OK
+    # the modular GEMMs keep the same promise: the raw-tile ring exists in the one-kernel form only
+    for tuning, want in ((dict(c_split=1, r_stages=2), vipir.ERR_UNSUPPORTED), (dict(c_split=2, r_stages=2), vipir.OK),
+                         (dict(r_stages=2), vipir.ERR_UNSUPPORTED)):  # 8 columns: the planner's form is two kernels
+        try:
+            vipir.ModGemmPlan(1, 2, 128, 128, 8, 0, [PRIMES[0]], tuning=tuning).close()
+            got = vipir.OK
+        except vipir.VipirError as e:
+            got = e.status
+        assert got == want, (tuning, got)
     with vipir.Plan(1024, 2048, 8, 8, None, M1, tuning=dict(m_sub=2, tile_queries=4, k_atoms=2, stages=3, min_chunks=4,
                                                             whole_units=1, no_collector=1)) as p:
         i = p.info
