@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- the VIPIR database scan on B200, measured.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--paper] [--modgemm] [--pipeline]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--paper] [--modgemm] [--pipeline] [--only NAME]
 
 Headline (BASELINE.json `metric`: "DB GB/s scanned & TOPS, % of HBM/INT8-TC roofline; 16 GiB u8
 DB, batch 1/256"): one STEP is one pass of the whole hot path -- query-limb split + scan (one
@@ -610,6 +610,14 @@ def run_cuda(args):
     vipir.load()
     peaks = measured_peaks()
 
+    if args.only:
+        # one named config alone (a BASELINE.json config or a --paper shape), e.g. as the target of an ncu capture:
+        # prints that config's measurements, not the bench line
+        r_, c_, _, bits_, _ = CONFIGS.get(args.only) or PAPER_CONFIGS[args.only]
+        buf = device.db(SEED, r_, c_, bits_).view(-1)
+        torch.cuda.synchronize()
+        print(json.dumps({"only": args.only, **run_config(args.only, buf, args.steps, args.warmup, peaks)}))
+        return
     rows, cols, _, _, _ = CONFIGS[HEADLINE]
     # this rank's row shard of the (world*rows) x cols DB: same stream, offset by the shard's first byte
     r0, _ = shard_rows(rank, world, rows)
@@ -841,6 +849,8 @@ def main():
                     help="also time the ring-packing stage at the paper's 64 GiB shape: lift + NTT (G, H) and H*C+(0|G)")
     ap.add_argument("--pipeline", action="store_true",
                     help="also time the built chain scan -> NTT -> H*C+(0|G) at the paper's 64 GiB hybrid shape")
+    ap.add_argument("--only", default=None, choices=sorted(list(CONFIGS) + list(PAPER_CONFIGS)),
+                    help="time this one config alone and print its measurements (N = 1; not the bench line)")
     ap.add_argument("--cpu-sample-rows", type=int, default=8192)
     ap.add_argument("--ref-sample-rows", type=int, default=8192)
     args = ap.parse_args()
