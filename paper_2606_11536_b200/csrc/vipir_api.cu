@@ -248,7 +248,8 @@ int plan_gemm(vipir_plan* p, int cg) {
     g.atom_bytes = msub * vipir::GM_A_BYTES + g.n_instr * (g.ni_cols / cg) * vipir::GM_BK;
     const uint32_t overhead = 1024 + 384;  // alignment slack + barriers (ring, accumulator, copier) and the words behind them
     // k-atoms per stage and ring depth (DESIGN.md section 6 "in-flight bytes")
-    // measured on B200 (profiles/r01_tuning.md): several k-atoms per stage (longer contiguous DB
+    // round-1 measurement on B200, not reproduced since (vipir_tuning.k_atoms / .stages reach the alternatives; round 3's
+    // configs[4] sweep, profiles/r03_ncu_gemm_i8_c5_planes.txt, again has k_atoms 2 behind the default): several k-atoms per stage (longer contiguous DB
     // runs per row, fewer barrier round trips) beat deeper rings of single atoms; keep >= 3 stages
     uint32_t katoms = (kMaxSmem - overhead) / 3 / g.atom_bytes;
     if (katoms > 4) katoms = 4;
@@ -433,7 +434,7 @@ int vipir_dbmul_plan_tuned(vipir_plan** out, uint64_t rows, uint64_t cols, uint3
 
     if (regime == VIPIR_REGIME_AUTO) {
         if (p->nq == 1 && n_moduli == 0 && !planes) regime = VIPIR_REGIME_GEMV;
-        // measured (profiles/r01_tuning.md): CTA pairs win from 32 query vectors up, where the limb
+        // round-1 measurement, not reproduced since (VIPIR_REGIME_MMA_1SM / _2SM force either): CTA pairs win from 32 query vectors up, where the limb
         // tile's shared-memory traffic starts to matter; below that one CTA per tile is as fast
         else regime = ((uint64_t)p->nq * p->lc > 64 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
     }
