@@ -39,7 +39,10 @@
  * that overlaps requests makes one plan per stream.  After one call outside the capture (which
  * sets kernel attributes and encodes the tensor maps for these buffers) a vipir_dbmul call can be
  * captured into a CUDA graph and replayed: the kernels reset their own work counters.  All
- * kernels are sm_100a; there is no fallback of any kind.
+ * kernels are sm_100a; there is no fallback of any kind.  A plan (of any of the three kinds in this header) belongs to
+ * the device that was current when it was made -- its workspace, tensor maps and streams live there -- and every call
+ * that takes it must come with that device current: under another one it returns VIPIR_ERR_INVALID_ARG and
+ * enqueues nothing (a process that drives several GPUs, makes one plan per GPU).
  *
  * Errors: every entry point returns a vipir_status (0 = OK) and never throws or aborts.
  */

@@ -11,6 +11,7 @@ struct vipir_modgemm_plan {
     uint32_t moduli[VIPIR_MAX_MODULI];
     vipir_modgemm_tuning tune;  // explicit planner overrides; all zero = the planner's own choices
     int num_sms;
+    int device;          // the device current at plan time: every call must come with it current
     uint8_t* d_hp;       // H byte limbs, interleaved per k-atom: [P*M][4*Kp]   (written by vipir_modgemm_set_h)
     uint8_t* d_cp;       // C limb planes: [P][4][ncols][Kp]                    (written every call)
     uint64_t hp_bytes, cp_bytes;
@@ -254,6 +255,7 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
     p->ncols = ncols;
     p->gcols = gcols;
     p->num_sms = sms;
+    p->device = dev;
     for (uint32_t t = 0; t < T; ++t) p->moduli[t] = moduli[t];
     if (tune) p->tune = *tune;
     // CTA pairs (one 256-row tile, each CTA staging half of the C limb tile) once the C tile is wide
@@ -296,6 +298,7 @@ int vipir_modgemm_plan_create_tuned(vipir_modgemm_plan** out, uint32_t T, uint64
 
 int vipir_modgemm_set_h(vipir_modgemm_plan* p, const uint32_t* d_H, void* cuda_stream) {
     if (!p || !d_H || (reinterpret_cast<uintptr_t>(d_H) & 15)) return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     int rc = launch_mg_split<true>(d_H, p->d_hp, p->P * p->M, p->M, p->K, p->Kp, static_cast<cudaStream_t>(cuda_stream));
     if (rc == VIPIR_OK) p->h_set = true;
     return rc;
@@ -303,6 +306,7 @@ int vipir_modgemm_set_h(vipir_modgemm_plan* p, const uint32_t* d_H, void* cuda_s
 
 int vipir_modgemm_split_c(vipir_modgemm_plan* p, const uint32_t* d_C, void* cuda_stream) {
     if (!p || !d_C || (reinterpret_cast<uintptr_t>(d_C) & 15)) return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     int rc = ensure_c_planes(p);
     if (rc != VIPIR_OK) return rc;
     return launch_mg_split<false>(d_C, p->d_cp, p->P * p->ncols, p->ncols, p->K, p->Kp,
@@ -314,6 +318,7 @@ int check_products_args(const vipir_modgemm_plan* p, const uint32_t* d_G, const 
     if (!p || !d_Out || (p->gcols > 0 && !d_G)) return VIPIR_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(d_Out) & 3) || (reinterpret_cast<uintptr_t>(d_G) & 3)) return VIPIR_ERR_INVALID_ARG;
     if (!p->h_set) return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     return VIPIR_OK;
 }
 }  // namespace

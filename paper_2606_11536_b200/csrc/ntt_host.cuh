@@ -9,6 +9,7 @@ struct vipir_ntt_plan {
     uint32_t T, log2n, N, p_bits, centered;
     uint32_t moduli[VIPIR_MAX_MODULI], scale[VIPIR_MAX_MODULI], scale_shoup[VIPIR_MAX_MODULI];
     int num_sms;
+    int device;            // the device current at plan time: every call must come with it current
     uint32_t* d_twiddles;  // [T][2][N]
     uint32_t* d_bad;       // device flag: an input word >= 2^p_bits was seen
 };
@@ -89,6 +90,7 @@ int vipir_ntt_plan_create(vipir_ntt_plan** out, uint32_t T, uint32_t log2n, cons
     p->p_bits = p_bits;
     p->centered = centered;
     p->num_sms = sms;
+    p->device = dev;
     std::vector<uint32_t> tab((size_t)T * 2 * N);
     for (uint32_t t = 0; t < T; ++t) {
         const uint32_t q = moduli[t];
@@ -125,6 +127,7 @@ int vipir_ntt_lift(vipir_ntt_plan* p, const uint32_t* d_X, uint32_t n_a, uint32_
     if (!p || !d_X || !d_O || n_a == 0 || M == 0 || out_layout > 1) return VIPIR_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(d_X) & 3) || (reinterpret_cast<uintptr_t>(d_O) & 3)) return VIPIR_ERR_INVALID_ARG;
     if ((uint64_t)n_a * M >= (1ull << 31)) return VIPIR_ERR_UNSUPPORTED;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     vipir::NttParams np{};
     np.T = p->T;
     if (out_layout == VIPIR_NTT_LAYOUT_G) {  // O[t][c][a][m]
@@ -153,6 +156,7 @@ int vipir_ntt_lift(vipir_ntt_plan* p, const uint32_t* d_X, uint32_t n_a, uint32_
 
 int vipir_ntt_bad_input(vipir_ntt_plan* p, uint32_t* seen) {
     if (!p || !seen) return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     // the flag is written by kernels on the caller's streams (possibly non-blocking ones, which the legacy
     // stream does not order against): wait for all of them before reading and clearing it
     CK(cudaDeviceSynchronize());

@@ -84,6 +84,13 @@ int make_tmap_2d(CUtensorMap* m, const void* base, CUtensorMapDataType dt, uint3
     return VIPIR_OK;
 }
 
+// A plan's workspace, tensor maps and streams belong to the device that was current when it was made: a call under
+// another current device would launch there against this device's addresses.  Checked on every call.
+bool on_device(int plan_device) {
+    int cur = -1;
+    return cudaGetDevice(&cur) == cudaSuccess && cur == plan_device;
+}
+
 uint32_t round_up(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
 uint32_t ceil_div(uint32_t x, uint32_t m) { return (x + m - 1) / m; }
 
@@ -100,6 +107,7 @@ struct vipir_plan {
     uint32_t db_signed;  // DB elements are two's-complement int8
     vipir_tuning tune;   // explicit planner overrides (vipir_dbmul_plan_tuned); all zero = the planner's own choices
     int num_sms;
+    int device;  // the device current at plan time: every call must come with it current
     // workspace
     uint8_t* d_planes;
     uint64_t planes_bytes;
@@ -430,6 +438,7 @@ int vipir_dbmul_plan_tuned(vipir_plan** out, uint64_t rows, uint64_t cols, uint3
     p->nq = T * batch;
     p->lc = (kdl == 2 && n_moduli > 0) ? 5u : 4u;  // split_limbs.cuh: the s = 4 column vanishes mod 2^32
     p->num_sms = sms;
+    p->device = dev;
     if (tune) p->tune = *tune;
 
     if (regime == VIPIR_REGIME_AUTO) {
@@ -471,6 +480,7 @@ int vipir_split_limbs(vipir_plan* p, const uint32_t* d_query, uint8_t* d_planes_
     if (!p || !d_query || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
         (reinterpret_cast<uintptr_t>(d_planes_out) & 15))
         return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     return launch_split(p, d_query, d_planes_out ? d_planes_out : p->d_planes, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -548,6 +558,7 @@ int vipir_dbmul_scan(vipir_plan* p, const void* d_db, uint32_t* d_answer, void* 
     if (!p || !d_db || !d_answer) return VIPIR_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_answer) & 3))
         return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     if (p->regime == VIPIR_REGIME_NAIVE) return VIPIR_ERR_UNSUPPORTED;  // the check kernel has no limb planes
     return scan_only(p, d_db, d_answer, static_cast<cudaStream_t>(cuda_stream));
 }
@@ -557,6 +568,7 @@ int vipir_dbmul(vipir_plan* p, const void* d_db, const uint32_t* d_query, uint32
     if ((reinterpret_cast<uintptr_t>(d_db) & 15) || (reinterpret_cast<uintptr_t>(d_query) & 15) ||
         (reinterpret_cast<uintptr_t>(d_answer) & 3))
         return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
 
     if (p->regime == VIPIR_REGIME_NAIVE) {
@@ -609,6 +621,7 @@ static uint32_t host_slices(const vipir_plan* p, size_t qbytes, uint32_t bounds[
 int vipir_dbmul_host(vipir_plan* p, const void* d_db, const uint32_t* h_query, uint32_t* h_answer, void* cuda_stream) {
     if (!p || !d_db || !h_query || !h_answer) return VIPIR_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(d_db) & 15) return VIPIR_ERR_INVALID_ARG;
+    if (!on_device(p->device)) return VIPIR_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t qbytes = (size_t)p->nq * p->cols * 4, abytes = (size_t)p->nq * p->rows * 4;
     if (!p->d_q_stage && cudaMalloc(&p->d_q_stage, qbytes) != cudaSuccess) {
@@ -904,6 +917,7 @@ extern "C" int vipir_dbmul_static(uint64_t rows, uint64_t cols, uint32_t batch, 
     pl.nq = nq;
     pl.lc = lc;
     pl.num_sms = sms;
+    pl.device = dev;
     pl.regime = ((uint64_t)nq * lc > 64 && rows > 128) ? VIPIR_REGIME_MMA_2SM : VIPIR_REGIME_MMA_1SM;
     pl.planes_bytes = planes_bytes;
     pl.d_sync = reinterpret_cast<uint32_t*>(scratch);

@@ -374,6 +374,30 @@ def test_tuning_overrides_are_honoured_or_refused():
         assert p.info["stages"] == 6 and p.info["launches"] == 2
 
 
+def test_plan_used_under_another_current_device_is_refused():
+    """A plan belongs to the device current at plan time (include/vipir.h); a call under another current device
+    returns INVALID_ARG and enqueues nothing.  Needs two GPUs: skipped on a one-GPU box."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    ensure_built()
+    D, Q = make(5, 256, 1024, 8)
+    with torch.cuda.device(0):
+        d_db = torch.from_numpy(D).cuda()
+        d_q = torch.from_numpy(Q.view(np.int32)).cuda()
+        d_a = torch.full((1, 8, 256), -1, dtype=torch.int32, device="cuda")
+        plan = vipir.Plan(256, 1024, 8)
+    with torch.cuda.device(1):
+        with pytest.raises(vipir.VipirError) as e:
+            plan(d_db, d_q, d_a, stream=0)
+        assert e.value.status == vipir.ERR_INVALID_ARG
+    with torch.cuda.device(0):
+        plan(d_db, d_q, d_a)
+        torch.cuda.synchronize()
+        assert_same(d_a.cpu().numpy().view(np.uint32), oracle.dbmul(D, Q))
+        plan.close()
+
+
 def test_auto_matches_oracle_on_config_1():
     # BASELINE.json configs[0]: D 1024x1024 u8, Q 1024x1 u32, q = 2^32, seed 0
     D, Q = make(0, 1024, 1024, 1)
@@ -580,6 +604,43 @@ def test_host_entry_point_random_shapes(seed):
     with plan:
         plan.host(d_db, h_q, h_a)
         assert_same(h_a.numpy().view(np.uint32), want)
+
+
+def test_host_and_device_entry_points_seeded_soak():
+    """A bounded soak in the suite (round 2's unbounded ones ran from working scripts and found the empty-chunk hang
+    pinned above): 160 seeded random shapes -- both tensor regimes, u8 / u16, 2^32 / primes, 1-4 K slices, forced extra
+    chunks, the fused switch -- each through vipir_dbmul_host into mapped memory AND vipir_dbmul, both against the
+    oracle.  A hang shows as the kernel's own trap or the test's timeout, a race as a wrong word."""
+    import torch
+    ensure_built()
+    rng = np.random.default_rng(20261106)
+    refused = 0
+    for case in range(160):
+        regime, bits, moduli, rows, cols, batch, tune, ms = _random_host_case(rng)
+        rows, batch = min(rows, 400), min(batch, 40)  # keeps the whole soak at a few seconds of oracle time
+        D, Q = make(5000 + case, rows, cols, batch, bits, moduli)
+        want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+        if ms:
+            want = oracle.modswitch(want, ms)
+        T = Q.shape[0]
+        d_db = torch.from_numpy(D.view(np.uint8).reshape(rows, -1)).cuda()
+        h_q = torch.from_numpy(Q.view(np.int32)).pin_memory()
+        h_a = torch.full((T, batch, rows), -1, dtype=torch.int32).pin_memory()
+        d_a = torch.full((T, batch, rows), -1, dtype=torch.int32, device="cuda")
+        try:
+            plan = vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, tuning=tune)
+        except vipir.VipirError as e:
+            assert e.status == vipir.ERR_UNSUPPORTED and "min_chunks" in tune, (case, tune, e)
+            refused += 1
+            continue
+        with plan:
+            plan.host(d_db, h_q, h_a)
+            plan(d_db, h_q.cuda(), d_a)
+            torch.cuda.synchronize()
+        what = f"case {case}: {rows}x{cols} B={batch} u{bits} {'primes' if moduli else '2^32'} regime {regime} {tune} ms={ms}"
+        assert np.array_equal(h_a.numpy().view(np.uint32), want), "host call, " + what
+        assert np.array_equal(d_a.cpu().numpy().view(np.uint32), want), "device call, " + what
+    assert refused < 40
 
 
 def test_two_plans_two_threads_two_streams():
