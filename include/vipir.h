@@ -114,6 +114,7 @@ typedef struct {
     uint32_t m_sub;           /* MMA regimes: 128-row DB sub-tiles per CTA and tile (rows per tile = 128 * CTAs * m_sub;
                                  LIMB_PLANES: the two limb tiles of a row block count as two sub-tiles) */
     uint32_t db_layout;       /* vipir_db_layout the plan expects d_db in */
+    uint32_t leftover_chunks; /* MMA: K chunks of a unit of the last, partial round (== n_chunks unless cut finer) */
 } vipir_info;
 
 /*
@@ -169,7 +170,11 @@ typedef struct {
                                 (no direct stores into mapped host memory, no overlapped copies) */
     uint32_t host_slices;    /* vipir_dbmul_host, MMA: K slices of the copy / split / scan pipeline, 1..4 (0: three for
                                 queries of 8 MiB and more, else one); UNSUPPORTED for a GEMV plan */
-    uint32_t reserved[6];    /* must be 0 */
+    uint32_t leftover_chunks; /* MMA: cut the units of the last, partial round (units mod CTA groups of them) into this many
+                                K chunks, so that the round can be dealt out evenly; >= the plan's n_chunks, <= k-atoms;
+                                UNSUPPORTED with whole_units.  0: the planner's rule (finer only where it shortens that
+                                round by a fifth or more) */
+    uint32_t reserved[5];    /* must be 0 */
 } vipir_tuning;
 
 /* vipir_dbmul_plan_layout with explicit planner overrides.  Errors: as vipir_dbmul_plan_layout; INVALID_ARG

@@ -44,7 +44,10 @@
 // one M tile run at the same time on neighbouring groups and share the DB tile through L2 --
 // and the units of the last, partial round are dealt out chunk by chunk in contiguous item
 // ranges, which removes the wave-quantisation loss (e.g. 256 units on 74 pairs: 3.5 rounds
-// instead of 4).  A unit split between two groups is accumulated through the answer buffer
+// instead of 4).  The leftover units may be cut into MORE chunks than the units of the full rounds
+// (GemmParams.nc_left: the planner's choice where few chunks would deal out badly, e.g. one chunk per unit),
+// which costs the extra accumulator drains only where they buy an even last round.
+// A unit split between two groups is accumulated through the answer buffer
 // (chunk 0 stores, later chunks add): the later group waits on a per-unit arrival counter in
 // global memory before its first read-modify-write.  Group ids are tickets drawn from an atomic
 // counter, a group only ever waits for lower tickets, and every group works through its
@@ -81,6 +84,8 @@ struct GemmParams {
     uint32_t total_ksteps;   // k-atoms of this launch's K range (ceil(K' / 128) for the whole product)
     uint32_t ksteps_per_chunk;
     uint32_t n_chunks;
+    uint32_t nc_left, kpc_left;  // units of the leftover round only: cut into nc_left chunks of kpc_left k-atoms instead
+                             // (finer items to deal out; 0 = like every other unit)
     uint32_t katoms;         // k-atoms per pipeline stage (>= 1): one stage = katoms x (A box + B boxes)
     uint32_t atom_bytes;     // per CTA: 16 KiB of DB + this CTA's share of the limb tile, for one k-atom
     uint32_t stages;
@@ -128,16 +133,16 @@ __device__ __forceinline__ uint32_t barrett_u64(uint64_t x, uint32_t p, uint64_t
 // the order  tail (chunks [0, c) of the range's last unit)  ->  whole units  ->  head (chunks
 // [c0, c1) of the range's first unit, whose earlier chunks belong to group g-1 or before).
 struct WorkPlan {
-    uint32_t g, G, nc, full_rounds, u_base;
+    uint32_t g, G, nc, nc_full, full_rounds, u_base;  // nc: chunks of a leftover unit; nc_full: of a unit of the full rounds
     uint32_t has_tail, tail_u, tail_c1;
     uint32_t mid0, mid1;
     uint32_t has_head, head_u, head_c0, head_c1;
 };
 
 __host__ __device__ __forceinline__ WorkPlan make_work_plan(uint32_t g, uint32_t G, uint32_t n_units, uint32_t nc,
-                                                   uint32_t split) {
+                                                   uint32_t split, uint32_t nc_full = 0) {
     WorkPlan w;
-    w.g = g; w.G = G; w.nc = nc;
+    w.g = g; w.G = G; w.nc = nc; w.nc_full = nc_full ? nc_full : nc;
     w.full_rounds = n_units / G;
     w.u_base = w.full_rounds * G;
     const uint32_t L = n_units - w.u_base;
@@ -175,7 +180,7 @@ __host__ __device__ __forceinline__ void for_each_item(const WorkPlan& w, F&& f)
     for (uint32_t seg = 0; seg < 4; ++seg) {
         uint32_t u_lo, u_hi, u_step = 1, c_lo = 0, c_hi = w.nc;
         if (seg == 0) {  // full rounds
-            u_lo = w.g; u_hi = w.u_base; u_step = w.G;
+            u_lo = w.g; u_hi = w.u_base; u_step = w.G; c_hi = w.nc_full;
         } else if (seg == 1) {  // tail of the leftover range: produces chunks another group continues
             u_lo = w.tail_u; u_hi = w.tail_u + w.has_tail; c_hi = w.tail_c1;
         } else if (seg == 2) {  // whole leftover units
@@ -256,7 +261,10 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     // teardown ends with a cluster barrier)
     const uint32_t ticket = __shfl_sync(
         0xffffffffu, (CG == 2 && rank == 1) ? ptx::ld_shared_cluster_u32(ticket_ptr, 0) : *ticket_ptr, 0);
-    const WorkPlan work = make_work_plan(ticket, p.n_groups, n_units, p.n_chunks, p.split);
+    // chunks of a unit: n_chunks x ksteps_per_chunk k-atoms in the full rounds; the leftover round's units may be cut finer
+    const uint32_t nc_left = p.nc_left ? p.nc_left : p.n_chunks;
+    const uint32_t kpc_left = p.nc_left ? p.kpc_left : p.ksteps_per_chunk;
+    const WorkPlan work = make_work_plan(ticket, p.n_groups, n_units, nc_left, p.split, p.n_chunks);
 
     if (warp == 0) {
         // ===== TMA producer: the whole warp runs the (warp-uniform) loop, one elected lane issues =====
@@ -275,8 +283,9 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 auto sub_row = [&](uint32_t j) {
                     return (int32_t)((j % NL) * p.rows + ((uint64_t)(mt * rsub + j / NL) * CG + rank) * GM_BM);
                 };
-                const uint32_t ks_begin = c * p.ksteps_per_chunk;
-                const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
+                const uint32_t kpc = (u < work.u_base) ? p.ksteps_per_chunk : kpc_left;
+                const uint32_t ks_begin = c * kpc;
+                const uint32_t ks_end = min(p.total_ksteps, ks_begin + kpc);
                 // a stage never straddles a chunk: the last stage of a chunk may hold fewer atoms
                 for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
                     const uint32_t na = min(p.katoms, ks_end - ks0);
@@ -324,15 +333,16 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (rank == 0) {
             uint32_t stage = 0, phase = 0, acc_it = 0;
             const uint32_t b_bytes = (p.ni_cols / CG) * GM_BK;
-            for_each_item(work, [&](uint32_t, uint32_t c, bool) {
+            for_each_item(work, [&](uint32_t u, uint32_t c, bool) {
                 const uint32_t as = acc_it % p.acc_stages;
                 const uint32_t aphase = (acc_it / p.acc_stages) & 1;
                 ++acc_it;
                 if constexpr (CG == 2) ptx::mbar_wait_cluster(&tmem_empty[as], aphase ^ 1);
                 else ptx::mbar_wait(&tmem_empty[as], aphase ^ 1);
                 ptx::tc_fence_after();
-                const uint32_t ks_begin = c * p.ksteps_per_chunk;
-                const uint32_t ks_end = min(p.total_ksteps, ks_begin + p.ksteps_per_chunk);
+                const uint32_t kpc = (u < work.u_base) ? p.ksteps_per_chunk : kpc_left;
+                const uint32_t ks_begin = c * kpc;
+                const uint32_t ks_end = min(p.total_ksteps, ks_begin + kpc);
                 const uint32_t tacc = tmem_base + as * acc_cols;
                 for (uint32_t ks0 = ks_begin; ks0 < ks_end; ks0 += p.katoms) {
                     const uint32_t na = min(p.katoms, ks_end - ks0);
@@ -396,8 +406,8 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const uint32_t cw = warp - 2;
         const bool vec = (p.rows % 4 == 0) && ((reinterpret_cast<uintptr_t>(p.answer) | reinterpret_cast<uintptr_t>(p.final_out)) & 15) == 0;
         uint32_t n_final = 0;
-        for_each_item(work, [&](uint32_t, uint32_t c, bool) {
-            if (c + 1 != p.n_chunks) return;
+        for_each_item(work, [&](uint32_t u_item, uint32_t c, bool) {
+            if (c + 1 != ((u_item < work.u_base) ? p.n_chunks : nc_left)) return;
             const uint32_t slot = n_final & 1, ph = (n_final >> 1) & 1;
             ++n_final;
             ptx::mbar_wait(&copy_full[slot], ph);
@@ -463,7 +473,7 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             // to round it: same batched prefetch, once per tile
             constexpr uint32_t kPf = 8;
             const bool first = c == 0 && !p.acc_in;   // nothing accumulated yet: plain store
-            const bool last = c + 1 == p.n_chunks;
+            const bool last = c + 1 == ((u < work.u_base) ? p.n_chunks : nc_left);
             const bool ms_final = !PRIME && p.ms_bits != 0 && last;
             const bool need_old = !first && (PRIME || ms_final);
             // every chunk lands in `answer`; when the result is wanted elsewhere (final_out: the host call's mapped

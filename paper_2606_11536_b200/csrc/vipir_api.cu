@@ -294,6 +294,37 @@ int plan_gemm(vipir_plan* p, int cg) {
     const uint64_t n_units64 = (uint64_t)g.m_tiles * g.n_tiles;
     g.n_groups = (uint32_t)(items < max_groups ? items : max_groups);
     if (!g.split && n_units64 < g.n_groups) g.n_groups = (uint32_t)n_units64;
+    // The last, partial round: L = units mod groups leftover units are dealt out chunk by chunk, so it takes
+    // ceil(L * nc / groups) / nc of a unit's time.  With few K chunks that rounds up badly (configs[4] as limb planes:
+    // 256 units of ONE chunk on 74 pairs = 34 pairs run a fourth unit while 40 idle, ncu: SMs active 84 % of the launch),
+    // so the leftover units alone may be cut finer; the units of the full rounds keep the fewest chunks (every extra chunk
+    // is one more accumulator drain).  Finer only where it shortens the round by a fifth or more, chunks of >= 8 KiB of K.
+    g.nc_left = g.kpc_left = 0;
+    {
+        uint32_t nc_left = 0;
+        if (const uint32_t force = p->tune.leftover_chunks) {
+            if (!g.split || force < g.n_chunks || force > g.total_ksteps) return VIPIR_ERR_UNSUPPORTED;
+            nc_left = force;
+        } else if (g.split && n_units64 > g.n_groups && n_units64 % g.n_groups != 0) {
+            const uint64_t L = n_units64 % g.n_groups;
+            auto cost = [&](uint32_t nc) { return (uint32_t)(((L * nc + g.n_groups - 1) / g.n_groups) * 1000 / nc); };
+            uint32_t best = g.n_chunks, best_cost = cost(g.n_chunks);
+            for (uint32_t mult = 2; mult <= 4; mult *= 2) {
+                const uint32_t kpc = ceil_div(g.total_ksteps, g.n_chunks * mult);
+                if (kpc < 64) break;
+                const uint32_t nc = ceil_div(g.total_ksteps, kpc);
+                if (cost(nc) * 10 <= best_cost * 8) best = nc, best_cost = cost(nc);
+            }
+            if (best != g.n_chunks) nc_left = best;
+        }
+        if (nc_left) {
+            const uint32_t kpc = ceil_div(g.total_ksteps, nc_left);
+            if (kpc != g.ksteps_per_chunk) {
+                g.kpc_left = kpc;
+                g.nc_left = ceil_div(g.total_ksteps, kpc);  // the chunks that exist (see n_chunks above)
+            }
+        }
+    }
     p->grid = g.n_groups * cg;
     if (!p->d_sync) {
         const size_t sync_bytes = (2 + (size_t)max_groups) * sizeof(uint32_t);
@@ -315,7 +346,8 @@ int plan_gemm(vipir_plan* p, int cg) {
 int plan_gemv(vipir_plan* p) {
     if (p->nq != 1 || p->n_moduli != 0 || p->lc != 4) return VIPIR_ERR_UNSUPPORTED;
     const vipir_tuning& tu = p->tune;  // overrides of the tensor-core regimes do not apply here
-    if (tu.m_sub || tu.tile_queries || tu.k_atoms || tu.min_chunks || tu.whole_units || tu.no_collector || tu.host_slices)
+    if (tu.m_sub || tu.tile_queries || tu.k_atoms || tu.min_chunks || tu.whole_units || tu.no_collector || tu.host_slices ||
+        tu.leftover_chunks)
         return VIPIR_ERR_UNSUPPORTED;
     vipir::GemvParams& g = p->gv;
     memset(&g, 0, sizeof g);
@@ -385,7 +417,8 @@ int vipir_dbmul_plan_tuned(vipir_plan** out, uint64_t rows, uint64_t cols, uint3
     if (tune) {  // domain of every field; whether the shape can honour it is the planner's UNSUPPORTED
         if ((tune->m_sub != 0 && tune->m_sub != 1 && tune->m_sub != 2 && tune->m_sub != 4) || tune->tile_queries > 128 ||
             tune->k_atoms > 8 || tune->stages == 1 || tune->stages > 12 || tune->separate_split > 1 ||
-            tune->whole_units > 1 || tune->no_collector > 1 || tune->host_staged > 1 || tune->host_slices > kMaxHostSlices)
+            tune->whole_units > 1 || tune->no_collector > 1 || tune->host_staged > 1 || tune->host_slices > kMaxHostSlices ||
+            tune->leftover_chunks > 4096)
             return VIPIR_ERR_INVALID_ARG;
         for (uint32_t r : tune->reserved)
             if (r != 0) return VIPIR_ERR_INVALID_ARG;
@@ -545,6 +578,7 @@ static int scan_only(vipir_plan* p, const void* d_db, uint32_t* d_answer, cudaSt
         g.total_ksteps = slice->k_atoms;
         g.n_chunks = ceil_div(slice->k_atoms, max_ksteps);
         g.ksteps_per_chunk = ceil_div(slice->k_atoms, g.n_chunks);
+        g.nc_left = g.kpc_left = 0;  // a K slice is short already: every unit in the same chunks
         g.acc_in = slice->acc_in;
         g.final_out = slice->final_out;
         if (!slice->is_last) g.ms_bits = 0;  // the switch rounds the complete sum only
@@ -765,6 +799,7 @@ int vipir_plan_info(const vipir_plan* p, vipir_info* o) {
     if (p->regime == VIPIR_REGIME_MMA_1SM || p->regime == VIPIR_REGIME_MMA_2SM) {
         o->k_chunk_bytes = p->gm.ksteps_per_chunk * vipir::GM_BK;
         o->n_chunks = p->gm.n_chunks;
+        o->leftover_chunks = p->gm.nc_left ? p->gm.nc_left : p->gm.n_chunks;
         o->tile_queries = p->gm.qt;
         o->tile_cols = p->gm.bn;
         o->mma_n = p->gm.ni_cols;

@@ -45,7 +45,7 @@ class Tuning(ctypes.Structure):
     _fields_ = [("m_sub", ctypes.c_uint32), ("tile_queries", ctypes.c_uint32), ("k_atoms", ctypes.c_uint32),
                 ("stages", ctypes.c_uint32), ("min_chunks", ctypes.c_uint32), ("separate_split", ctypes.c_uint32),
                 ("whole_units", ctypes.c_uint32), ("no_collector", ctypes.c_uint32), ("host_staged", ctypes.c_uint32),
-                ("host_slices", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 6)]
+                ("host_slices", ctypes.c_uint32), ("leftover_chunks", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 5)]
 
 
 class ModGemmTuning(ctypes.Structure):
@@ -64,7 +64,7 @@ class Info(ctypes.Structure):
         ("stages", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32), ("grid", ctypes.c_uint32),
         ("launches", ctypes.c_uint32), ("workspace_bytes", ctypes.c_uint64),
         ("modswitch_bits", ctypes.c_uint32), ("db_signed", ctypes.c_uint32), ("m_sub", ctypes.c_uint32),
-        ("db_layout", ctypes.c_uint32),
+        ("db_layout", ctypes.c_uint32), ("leftover_chunks", ctypes.c_uint32),
     ]
 
     def as_dict(self):

@@ -553,6 +553,51 @@ def test_host_entry_point_at_scale_planner_slices_several_units_per_cta():
     assert np.array_equal(d_a.cpu().numpy().view(np.uint32), got), "host and device entry points differ"
 
 
+@pytest.mark.parametrize("name,regime,rows,cols,batch,bits,moduli,layout,tune,ms", [
+    ("M2 one chunk -> 3", M2, 24000, 2064, 24, 8, None, vipir.DB_ROW_MAJOR, dict(m_sub=1, leftover_chunks=3), 0),
+    ("M1 primes one chunk -> 4", M1, 24000, 4112, 8, 8, PRIMES, vipir.DB_ROW_MAJOR, dict(m_sub=1, leftover_chunks=4), 0),
+    ("M2 limb planes primes -> 2", M2, 20000, 1040, 12, 16, PRIMES, vipir.DB_LIMB_PLANES, dict(leftover_chunks=2), 0),
+    ("M2 two chunks -> 5, switch", M2, 24000, 40000, 8, 8, None, vipir.DB_ROW_MAJOR, dict(m_sub=1, leftover_chunks=5), 18),
+    ("M2 u16 byte view primes -> 3", M2, 20000, 1032, 8, 16, PRIMES, vipir.DB_ROW_MAJOR, dict(m_sub=1, leftover_chunks=3), 0),
+])
+def test_leftover_round_cut_into_finer_chunks(name, regime, rows, cols, batch, bits, moduli, layout, tune, ms):
+    """More units than CTA groups, and the units of the last, partial round cut into more K chunks than those of the
+    full rounds (vipir_tuning.leftover_chunks; the planner does this by itself for configs[4] held as limb planes):
+    device call in full against the oracle, and the K-sliced host call of the same plan (its slices use uniform
+    chunks) equal to it."""
+    import torch
+    D, Q = make(61, rows, cols, batch, bits, moduli)
+    want = oracle.dbmul(D, Q, moduli, nthreads=NT)
+    if ms:
+        want = oracle.modswitch(want, ms)
+    got, info = run_dbmul(D, Q, moduli, regime, return_info=True, modswitch_bits=ms, db_layout=layout, tuning=tune)
+    groups = info["grid"] // (2 if regime == M2 else 1)
+    assert info["m_tiles"] * info["n_tiles"] > groups and (info["m_tiles"] * info["n_tiles"]) % groups != 0, info
+    assert info["leftover_chunks"] == tune["leftover_chunks"] > info["n_chunks"], info
+    assert_same(got, want)
+    if layout == vipir.DB_ROW_MAJOR:
+        T = Q.shape[0]
+        d_db = torch.from_numpy(D.view(np.uint8).reshape(rows, -1)).cuda()
+        h_a = torch.full((T, batch, rows), -1, dtype=torch.int32).pin_memory()
+        with vipir.Plan(rows, cols, batch, bits, moduli, regime, ms, tuning=dict(tune, host_slices=2)) as plan:
+            plan.host(d_db, torch.from_numpy(Q.view(np.int32)).pin_memory(), h_a)
+        assert_same(h_a.numpy().view(np.uint32), want)
+
+
+def test_leftover_chunks_planner_rule_and_refusals():
+    ensure_built()
+    # configs[4] as limb planes: 256 one-chunk units on 74 pairs -> the 34 leftover units are cut in two (3.5 rounds, not 4)
+    with vipir.Plan(32768, 32768, 64, 16, PRIMES[:2], db_layout=vipir.DB_LIMB_PLANES) as p:
+        assert (p.info["n_chunks"], p.info["leftover_chunks"], p.info["m_tiles"] * p.info["n_tiles"], p.info["grid"]) == (1, 2, 256, 148)
+    # configs[3]: 68 leftover units of two chunks on 74 pairs -- no finer cut shortens that round
+    with vipir.Plan(65536, 65536, 256) as p:
+        assert p.info["leftover_chunks"] == p.info["n_chunks"] == 2
+    for tune in (dict(leftover_chunks=1, min_chunks=2), dict(leftover_chunks=2, whole_units=1), dict(leftover_chunks=17)):
+        with pytest.raises(vipir.VipirError) as e:  # fewer than n_chunks; nothing is split; more than the 16 k-atoms
+            vipir.Plan(1024, 2048, 8, 8, None, M1, tuning=tune)
+        assert e.value.status == vipir.ERR_UNSUPPORTED, tune
+
+
 def test_forced_chunk_count_that_does_not_divide_the_k_atoms():
     """6 k-atoms cut into "4" chunks are three chunks of two (a fourth, empty chunk would never complete: this shape
     hung the kernel until the planner counted the chunks that exist).  Found by a random soak of the host call."""
